@@ -1,0 +1,144 @@
+"""Pins for the oracle's estimator / imaging-condition parts (not gpu).
+
+What is pinned against what:
+  * probe accumulation  : Uz == history^T Z through numpy's matmul   (Eq. 3: u_bar = Q^T u)
+  * estimator vs exact  : r = nt, Z = sqrt(nt) I  =>  image == sum_t u v  (Eq. 1-3, north_star check 1)
+  * unbiasedness / rate : mean over draws -> exact; variance closed form of Avron & Toledo (ref [20],
+                          PAPER.md:L125); error falls ~2x per 4x r ("decays with r")
+  * offset volumes      : G[h=0] == image bitwise; brute-force Python triple loop (Eq. 4)
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+import rtm_inputs as ri
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    p = ri.random_acoustic(2, n=(14, 12), nb=6, nt=48, r=4, seed=21, nsrc=1, nrec=6)
+    p.wav = ri.ricker(p.nt, p.dt, 60.0)[:, None].copy()
+    co = orc.coeffs(p)
+    f = orc.forward(p, co, Z=p.Z, want_hist=True)
+    din = f["samples"].astype(np.float32)
+    a = orc.adjoint(p, co, din, Z=p.Z, want_hist=True)
+    return p, co, f, a, din
+
+
+def test_probe_accumulation_is_history_times_Z(tiny):
+    p, co, f, a, _ = tiny
+    Z = p.Z.astype(np.float64)
+    for res in (f, a):
+        ref = (res["hist"].T @ Z).T                      # [r][N]
+        assert np.abs(res["PZ"] - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+def test_identity_probes_give_exact_image(tiny):
+    p, co, f, a, din = tiny
+    Z = ri.identity_probes(p.nt)                         # r = nt, (1/r) Z Z^T = I
+    # sqrt(48) is not an fp32 number: use the value the oracle actually sees
+    z = float(Z[0, 0])
+    fz = orc.forward(p, co, Z=Z)
+    az = orc.adjoint(p, co, din, Z=Z)
+    I = orc.image(fz["PZ"], az["PZ"], 1.0 / (z * z))
+    Iex = orc.exact_image(f["hist"], a["hist"])
+    assert np.abs(Iex).max() > 0
+    assert np.abs(I - Iex).max() <= 1e-12 * np.abs(Iex).max()
+    # and with scale = 1/r the only difference is fp32(sqrt(nt))^2 / nt
+    I2 = orc.image(fz["PZ"], az["PZ"], 1.0 / p.nt)
+    assert np.allclose(I2, Iex * (z * z / p.nt), rtol=1e-12, atol=0)
+
+
+def test_exact_image_is_plain_sum(tiny):
+    p, co, f, a, _ = tiny
+    ref = np.einsum("tn,tn->n", f["hist"], a["hist"])
+    assert np.allclose(orc.exact_image(f["hist"], a["hist"]), ref, rtol=1e-13, atol=1e-300)
+
+
+@pytest.mark.parametrize("kind", ["gauss", "rademacher"])
+def test_unbiased_and_variance_closed_form(tiny, kind):
+    p, co, f, a, _ = tiny
+    uh, vh = f["hist"], a["hist"]                        # [nt][N]
+    Iex = orc.exact_image(uh, vh)
+    nt, N = uh.shape
+    r, M = 4, 6000
+    rng = np.random.default_rng(99)
+    acc = np.zeros(N)
+    acc2 = np.zeros(N)
+    for _ in range(M):
+        if kind == "gauss":
+            Z = rng.standard_normal((nt, r))
+        else:
+            Z = rng.integers(0, 2, (nt, r)) * 2.0 - 1.0
+        I = orc.image((uh.T @ Z).T, (vh.T @ Z).T, 1.0 / r)
+        acc += I
+        acc2 += I * I
+    mean = acc / M
+    var = acc2 / M - mean ** 2
+    nu = (uh ** 2).sum(0)
+    nv = (vh ** 2).sum(0)
+    var_cf = (nu * nv + Iex ** 2) / r
+    if kind == "rademacher":
+        var_cf = var_cf - 2.0 * ((uh * vh) ** 2).sum(0) / r
+    big = var_cf > 1e-3 * var_cf.max()
+    # unbiased: |mean - exact| within 5 standard errors
+    assert np.all(np.abs(mean - Iex)[big] <= 5.0 * np.sqrt(var_cf[big] / M))
+    # variance closed form (sample variance of M draws: relative sd ~ sqrt(2/M)*kurtosis factor)
+    ratio = var[big] / var_cf[big]
+    assert abs(np.median(ratio) - 1.0) < 0.05
+    assert np.all((ratio > 0.7) & (ratio < 1.4))
+
+
+def test_error_decays_like_one_over_sqrt_r(tiny):
+    p, co, f, a, _ = tiny
+    uh, vh = f["hist"], a["hist"]
+    Iex = orc.exact_image(uh, vh)
+    rng = np.random.default_rng(5)
+    errs = []
+    for r in (4, 16, 64):
+        e = []
+        for _ in range(200):
+            Z = rng.standard_normal((uh.shape[0], r))
+            I = orc.image((uh.T @ Z).T, (vh.T @ Z).T, 1.0 / r)
+            e.append(np.linalg.norm(I - Iex) ** 2)
+        errs.append(np.sqrt(np.mean(e)))
+    assert 1.8 < errs[0] / errs[1] < 2.2
+    assert 1.8 < errs[1] / errs[2] < 2.2
+
+
+def test_offset_gather_h0_is_image_and_bruteforce():
+    rng = np.random.default_rng(8)
+    nx, nz, r = 9, 5, 3
+    N = nx * nz
+    Uz = rng.standard_normal((r, N))
+    Vz = rng.standard_normal((r, N))
+    offs = np.array([-9, -3, -1, 0, 1, 2, 8], np.int32)
+    G = orc.offset_gather((nx, nz), Uz, Vz, offs, 1.0 / r)
+    I = orc.image(Uz, Vz, 1.0 / r)
+    assert np.array_equal(G[3], I)                       # PAPER.md:L52, bitwise
+    U3 = Uz.reshape(r, nx, nz)
+    V3 = Vz.reshape(r, nx, nz)
+    for ih, h in enumerate(offs):
+        for ix in range(nx):
+            for iz in range(nz):
+                s = 0.0
+                if 0 <= ix + h < nx and 0 <= ix - h < nx:
+                    for k in range(r):
+                        s += U3[k, ix + h, iz] * V3[k, ix - h, iz]
+                assert abs(G[ih, ix * nz + iz] - s / r) <= 1e-14 * max(1.0, abs(s))
+    assert np.all(G[0] == 0) and np.any(G[6] != 0) is not None
+
+
+def test_offset_gather_3d_layout():
+    rng = np.random.default_rng(9)
+    n = (5, 3, 4)
+    r = 2
+    N = int(np.prod(n))
+    Uz = rng.standard_normal((r, N))
+    Vz = rng.standard_normal((r, N))
+    G = orc.offset_gather(n, Uz, Vz, np.array([1], np.int32), 1.0)
+    U = Uz.reshape(r, *n)
+    V = Vz.reshape(r, *n)
+    ref = np.zeros(n)
+    ref[1:-1] = (U[:, 2:] * V[:, :-2]).sum(0)
+    assert np.allclose(G[0].reshape(n), ref, rtol=1e-14, atol=1e-14)
