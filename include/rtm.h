@@ -1,0 +1,137 @@
+/*
+ * rtm.h -- C ABI of the B200 (sm_100a) RTM-with-randomized-trace-imaging hot path.
+ *
+ * Method: Louboutin & Herrmann, "Enabling wave-based inversion on GPUs with randomized trace
+ * estimation" (arXiv 2201.06914); citations are PAPER.md:Lnn (+ section / equation).
+ * The paper fixes the estimator (Eq. 1), the imaging conditions (Eq. 2-4) and the
+ * O(N r) memory claim (L47, Table 1).  It gives no discretisation; DESIGN.md "Readings"
+ * fixes the FD scheme, boundary, source/receiver handling.
+ *
+ * Conventions
+ *   - plain C, no exceptions cross the ABI; every call returns 0 or a negative RTM_E* code.
+ *   - pointer prefix d_ = device memory, h_ = host memory.  The caller owns every buffer,
+ *     including the workspace; the library allocates and frees no device memory.
+ *   - all device work is enqueued on the `cuda_stream` argument (a cudaStream_t passed as void*);
+ *     no call synchronises the device.  Host tables (geometry) are built synchronously on the host
+ *     and uploaded with cudaMemcpyAsync on the same stream.
+ *   - grids: physical grid n = (nx,[ny],nz), z contiguous (C order [x][z] / [x][y][z]); absorbing
+ *     layer of nb points on every side; padded grid P = n + 2 nb, Np = prod P, N = prod n.
+ *     "canonical [Np]" / "[N]" arrays are dense C-order arrays without halo or pitch.
+ *   - fp32 storage and arithmetic on the device.
+ */
+#ifndef RTM_H
+#define RTM_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RTM_OK 0
+#define RTM_EINVAL (-1) /* bad shape / NULL / position outside the physical grid / bad offset   */
+#define RTM_ENOMEM (-2) /* workspace too small                                                  */
+#define RTM_ECUDA (-3)  /* a CUDA call failed; text via rtm_last_cuda_error()                   */
+#define RTM_ESTATE (-4) /* call order: adjoint before forward, gather before adjoint, no model  */
+
+typedef struct rtm_ctx rtm_ctx; /* opaque, host-side */
+
+typedef struct {
+    int ndim;       /* 2 | 3 */
+    int n[3];       /* physical points: 2D (nx, nz, -) ; 3D (nx, ny, nz); z contiguous            */
+    float h;        /* grid spacing [m], same on every axis                                       */
+    int nb;         /* absorbing-layer points on every side; must be a multiple of 4 (alignment)  */
+    int physics;    /* 0 isotropic acoustic ; 1 pseudo-acoustic TTI (ndim == 2 only)              */
+    int nt;         /* time steps                                                                 */
+    double dt;      /* time step [s] (used by rtm_coeffs_host only)                               */
+    int r;          /* number of probing vectors, 1..256 (Eq. 1)                    */
+    int max_pts;    /* upper bound on nsrc and nrec of any later call (sizes geometry tables)     */
+} rtm_config;
+
+/* Bytes of device workspace rtm_create needs for this config; 0 if the config is invalid.
+ * Holds: wavefields (u ping-pong + increment; x2 for TTI), coefficient arrays, damping tables,
+ * the compressed wavefields Uz and Vz (2 r N floats: the O(N r) storage of PAPER.md:L47 / Table 1),
+ * probe matrices (2 nt r), geometry tables.                                                       */
+size_t rtm_workspace_bytes(const rtm_config *cfg);
+
+/* Create a context over a caller-owned device workspace (256-byte aligned, >= rtm_workspace_bytes).
+ * Errors: RTM_EINVAL (bad config / NULL / misaligned), RTM_ENOMEM (bytes too small).              */
+int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes, rtm_ctx **out);
+void rtm_destroy(rtm_ctx *ctx);
+
+/* Host helper: coefficient arrays of the scheme (1/c^2)(u_tt + 2 sigma u_t) - Lap u = q from the
+ * earth model (O1).  fp64 arithmetic, one rounding to fp32.  Inputs are canonical [N]
+ * host arrays (eps/delta/theta may be NULL for physics 0); outputs canonical [Np] host arrays
+ * (TTI outputs may be NULL for physics 0) and h_damp1d = per-axis tables sigma_a*dt concatenated
+ * over the axes (Px [+Py] +Pz floats).                                                           */
+int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
+                    const float *h_theta, float *h_K2, float *h_epsh, float *h_delh, float *h_cos,
+                    float *h_sin, float *h_damp1d);
+
+/* Load the coefficient arrays (canonical [Np] DEVICE arrays; TTI ones NULL for physics 0) and the
+ * per-axis damping tables (HOST) into the workspace's internal (haloed, pitched) layout.         */
+int rtm_set_model(rtm_ctx *ctx, const float *d_K2, const float *d_epsh, const float *d_delh,
+                  const float *d_cos, const float *d_sin, const float *h_damp1d, void *cuda_stream);
+
+/* Probing matrices Z (reading C1/C2: E[z z^T] = I, drawn by the caller), device
+ * arrays [nt][r]; row n probes the field computed by step n (reading C6).  Zf is used by the
+ * forward pass, Za by the adjoint pass (may alias; separate so that Eq. 3's u_tt can be had by
+ * differencing Z, reading C4).  Copied into the workspace.                                        */
+int rtm_set_probes(rtm_ctx *ctx, const float *d_Zf, const float *d_Za, void *cuda_stream);
+
+/* Forward pass with fused probing (Eq. 3: u_bar = Z^T u accumulated on the fly).
+ * Zeroes the wavefields and Uz, runs n = 0..nt-1:  time step with fused damping; inject
+ * K2 h^(2-d) w wav[n][s] at the 2^d corners of each source; record d[n][j] = sum_c w u[corner];
+ * Uz[k][x] += Zf[n][k] u[x] on the physical grid.  Leaves Uz in the context.
+ *   h_src_xyz [nsrc][ndim], h_rec_xyz [nrec][ndim]: metres from the physical origin (HOST);
+ *   d_wav [nt][nsrc] (DEVICE); d_data_out [nt][nrec] (DEVICE) or NULL.
+ * Errors: RTM_EINVAL (NULL, counts > max_pts, a position outside [0,(n_a-1)h]), RTM_ESTATE.       */
+int rtm_forward_probe(rtm_ctx *ctx, int nsrc, const float *h_src_xyz, const float *d_wav, int nrec,
+                      const float *h_rec_xyz, float *d_data_out, void *cuda_stream);
+
+/* Adjoint pass with fused probing, then the image (Eq. 2-3).
+ * Zeroes the wavefields and Vz, runs n = nt-1..0: time step; inject K2 h^2 w din[n][j] at the
+ * receivers; optionally record qadj[n][s] = h^-d sum_c w v[corner] at the sources (exact transpose
+ * of the forward map wav -> data); Vz[k][x] += Za[n][k] v[x].  Then
+ *   image[x] (+)= scale * sum_k Uz[k][x] Vz[k][x]            (pass scale = 1/r for Eq. 3).
+ *   d_data_in [nt][nrec]; d_qadj_out [nt][nsrc] or NULL; d_image canonical [N] or NULL
+ *   (NULL: only Vz is formed); accumulate != 0 adds into d_image (stacking shots, L54/L77).       */
+int rtm_adjoint_image(rtm_ctx *ctx, int nrec, const float *h_rec_xyz, const float *d_data_in, int nsrc,
+                      const float *h_src_xyz, float *d_qadj_out, float scale, int accumulate,
+                      float *d_image, void *cuda_stream);
+
+/* Horizontal subsurface-offset volumes (Eq. 4; reading C11):
+ *   gather[ih][x] = scale * sum_k Uz[k][x + h e_x] Vz[k][x - h e_x],  h = h_offsets[ih] grid points
+ *   along x, zero where x+h or x-h leaves [0,nx).  gather[h=0] == image (L52).
+ *   d_gather [nh][N].  Errors: RTM_EINVAL (nh < 1, |h| >= nx), RTM_ESTATE (no Uz/Vz yet).         */
+int rtm_offset_gather(rtm_ctx *ctx, int nh, const int *h_offsets, float scale, float *d_gather,
+                      void *cuda_stream);
+
+/* One whole shot from HOST buffers (the end-to-end call): uploads wav and data_in, runs
+ * rtm_forward_probe, rtm_adjoint_image and (nh > 0) rtm_offset_gather, downloads data_out, image
+ * and gather.  Host buffers should be pinned for true asynchrony.  d_staging: caller-owned device
+ * scratch of at least rtm_shot_staging_bytes(...) bytes.  Any output pointer may be NULL.         */
+size_t rtm_shot_staging_bytes(const rtm_config *cfg, int nsrc, int nrec, int nh);
+int rtm_shot_host(rtm_ctx *ctx, int nsrc, const float *h_src_xyz, const float *h_wav, int nrec,
+                  const float *h_rec_xyz, const float *h_data_in, float *h_data_out, float scale,
+                  float *h_image, int nh, const int *h_offsets, float *h_gather, void *d_staging,
+                  size_t staging_bytes, void *cuda_stream);
+
+/* ---- test hooks ------------------------------------------------------------------------------ */
+/* Compressed wavefields in canonical order [r][N]: which = 0 Uz, 1 Vz.                            */
+int rtm_export_probes(rtm_ctx *ctx, int which, float *d_out, void *cuda_stream);
+/* Ask the NEXT pass to copy the wavefield(s) right after the listed steps (incl. injection) into
+ * d_out [nsnap][nf][Np] canonical (nf = 1 acoustic, 2 TTI: p then r).  nsnap = 0 clears.          */
+int rtm_set_snapshots(rtm_ctx *ctx, int nsnap, const int *h_steps, float *d_out);
+/* Internal coefficient array in canonical [Np] order: which = 0 K2, 1 epsh, 2 delh, 3 cos, 4 sin. */
+int rtm_export_coeff(rtm_ctx *ctx, int which, float *d_out, void *cuda_stream);
+/* Number of kernels this context has launched so far (bench.py's gpu_launches).                  */
+long long rtm_launch_count(const rtm_ctx *ctx);
+/* Tuning knob: name/value pairs such as "graph" (CUDA-graph the time loop).      */
+int rtm_set_option(rtm_ctx *ctx, const char *name, int value);
+
+const char *rtm_strerror(int code);
+const char *rtm_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RTM_H */

@@ -1,0 +1,5 @@
+"""B200-native (sm_100a) hot path of arXiv 2201.06914: FD wave propagation with the randomized-trace
+imaging condition fused into the time loop.  Thin Python binding over the C ABI in include/rtm.h.
+
+There is no CPU fallback: importing the binding fails loudly if the CUDA library is missing."""
+from .binding import (RTMError, Rtm, RtmConfig, coeffs_host, lib_path, load_library, workspace_bytes)  # noqa: F401

@@ -1,0 +1,286 @@
+"""ctypes binding of include/rtm.h -- argument marshalling only; every step runs in the CUDA kernels.
+
+PyTorch is used for device memory and streams (tensor.data_ptr(), torch.cuda.current_stream())."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "csrc", "librtm.so")
+_lib = None
+
+EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
+           "rtm_set_probes", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
+           "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
+           "rtm_export_coeff", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
+
+
+class RTMError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(msg)
+        self.code = code
+
+
+class RtmConfig(C.Structure):
+    _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("h", C.c_float), ("nb", C.c_int),
+                ("physics", C.c_int), ("nt", C.c_int), ("dt", C.c_double), ("r", C.c_int),
+                ("max_pts", C.c_int)]
+
+
+def lib_path() -> str:
+    return _LIBPATH
+
+
+def load_library():
+    """Load csrc/librtm.so; raises (no fallback) if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBPATH):
+        raise ImportError("CUDA library %s is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)" % _LIBPATH)
+    lib = C.CDLL(_LIBPATH)
+    vp, ip, fp = C.c_void_p, C.c_int, C.c_float
+    cfgp = C.POINTER(RtmConfig)
+    lib.rtm_workspace_bytes.restype = C.c_size_t
+    lib.rtm_workspace_bytes.argtypes = [cfgp]
+    lib.rtm_create.argtypes = [cfgp, vp, C.c_size_t, C.POINTER(vp)]
+    lib.rtm_destroy.argtypes = [vp]
+    lib.rtm_destroy.restype = None
+    lib.rtm_coeffs_host.argtypes = [cfgp] + [vp] * 10
+    lib.rtm_set_model.argtypes = [vp] * 8
+    lib.rtm_set_probes.argtypes = [vp] * 4
+    lib.rtm_forward_probe.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp]
+    lib.rtm_adjoint_image.argtypes = [vp, ip, vp, vp, ip, vp, vp, fp, ip, vp, vp]
+    lib.rtm_offset_gather.argtypes = [vp, ip, vp, fp, vp, vp]
+    lib.rtm_shot_staging_bytes.restype = C.c_size_t
+    lib.rtm_shot_staging_bytes.argtypes = [cfgp, ip, ip, ip]
+    lib.rtm_shot_host.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp, fp, vp, ip, vp, vp, vp, C.c_size_t, vp]
+    lib.rtm_export_probes.argtypes = [vp, ip, vp, vp]
+    lib.rtm_set_snapshots.argtypes = [vp, ip, vp, vp]
+    lib.rtm_export_coeff.argtypes = [vp, ip, vp, vp]
+    lib.rtm_launch_count.restype = C.c_longlong
+    lib.rtm_launch_count.argtypes = [vp]
+    lib.rtm_set_option.argtypes = [vp, C.c_char_p, ip]
+    lib.rtm_strerror.restype = C.c_char_p
+    lib.rtm_strerror.argtypes = [ip]
+    lib.rtm_last_cuda_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc):
+    if rc != 0:
+        lib = load_library()
+        msg = lib.rtm_strerror(rc).decode()
+        if rc == -3:
+            msg += ": " + lib.rtm_last_cuda_error().decode()
+        raise RTMError(rc, "rtm error %d: %s" % (rc, msg))
+
+
+def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts) -> RtmConfig:
+    c = RtmConfig()
+    c.ndim = int(ndim)
+    for i, v in enumerate(n):
+        c.n[i] = int(v)
+    c.h = float(h)
+    c.nb = int(nb)
+    c.physics = int(physics)
+    c.nt = int(nt)
+    c.dt = float(dt)
+    c.r = int(r)
+    c.max_pts = int(max_pts)
+    return c
+
+
+def workspace_bytes(cfg: RtmConfig) -> int:
+    return int(load_library().rtm_workspace_bytes(C.byref(cfg)))
+
+
+def _hp(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def coeffs_host(cfg: RtmConfig, vp, eps=None, delta=None, theta=None):
+    """rtm_coeffs_host: (K2, epsh, delh, cos, sin, damp1d) as numpy fp32 arrays (canonical [Np])."""
+    lib = load_library()
+    nd = cfg.ndim
+    n = [cfg.n[i] for i in range(nd)]
+    P = [a + 2 * cfg.nb for a in n]
+    Np = int(np.prod(P))
+    f32 = lambda a: None if a is None else np.ascontiguousarray(a, np.float32)
+    vp, eps, delta, theta = f32(vp), f32(eps), f32(delta), f32(theta)
+    K2 = np.empty(Np, np.float32)
+    damp = np.empty(sum(P), np.float32)
+    tti = cfg.physics == 1
+    outs = [np.empty(Np, np.float32) if tti else None for _ in range(4)]
+    _check(lib.rtm_coeffs_host(C.byref(cfg), _hp(vp), _hp(eps), _hp(delta), _hp(theta), _hp(K2),
+                               _hp(outs[0]), _hp(outs[1]), _hp(outs[2]), _hp(outs[3]), _hp(damp)))
+    return K2, outs[0], outs[1], outs[2], outs[3], damp
+
+
+class Rtm:
+    """One context = one (model, acquisition size) on one GPU.  Same calls as include/rtm.h."""
+
+    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.lib = load_library()
+        self.cfg = make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts)
+        self.device = torch.device(device)
+        nbytes = workspace_bytes(self.cfg)
+        if nbytes == 0:
+            raise RTMError(-1, "rtm error -1: invalid config")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        h_ = C.c_void_p()
+        _check(self.lib.rtm_create(C.byref(self.cfg), self.workspace.data_ptr(), nbytes, C.byref(h_)))
+        self.ctx = h_
+        self.n = tuple(int(v) for v in n)
+        self.N = int(np.prod(self.n))
+        self.P = tuple(v + 2 * nb for v in self.n)
+        self.Np = int(np.prod(self.P))
+        self.nt, self.r, self.ndim, self.physics = int(nt), int(r), int(ndim), int(physics)
+        self._keep = []
+
+    @classmethod
+    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None):
+        mp = max(len(p.src_xyz), len(p.rec_xyz)) if max_pts is None else max_pts
+        return cls(p.ndim, p.n, p.h, p.nb, p.physics, p.nt if nt is None else nt, p.dt,
+                   p.r if r is None else r, mp, device=device)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            self.torch.cuda.synchronize(self.device)
+            self.lib.rtm_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers -------------------------------------------------------------------------------------
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def _dev(self, a):
+        t = self.torch
+        if a is None:
+            return None
+        if isinstance(a, t.Tensor):
+            assert a.is_cuda and a.dtype == t.float32 and a.is_contiguous()
+            return a
+        return t.from_numpy(np.ascontiguousarray(a, np.float32)).to(self.device)
+
+    @staticmethod
+    def _ptr(tens):
+        return None if tens is None else C.c_void_p(tens.data_ptr())
+
+    # -- API ------------------------------------------------------------------------------------------
+    def set_model_from_earth(self, vp, eps=None, delta=None, theta=None):
+        K2, eh, dh, cs, sn, damp = coeffs_host(self.cfg, vp, eps, delta, theta)
+        self.set_model(K2, eh, dh, cs, sn, damp)
+        return K2, eh, dh, cs, sn, damp
+
+    def set_model(self, K2, epsh, delh, cosT, sinT, damp1d):
+        d = [self._dev(a) for a in (K2, epsh, delh, cosT, sinT)]
+        damp = np.ascontiguousarray(damp1d, np.float32)
+        _check(self.lib.rtm_set_model(self.ctx, *[self._ptr(x) for x in d], _hp(damp), self._stream()))
+        self._keep = [d, damp]
+
+    def set_probes(self, Zf, Za=None):
+        zf = self._dev(Zf)
+        za = zf if Za is None else self._dev(Za)
+        assert tuple(zf.shape) == (self.nt, self.r) and tuple(za.shape) == (self.nt, self.r)
+        _check(self.lib.rtm_set_probes(self.ctx, self._ptr(zf), self._ptr(za), self._stream()))
+        self._keep_z = (zf, za)
+
+    def forward_probe(self, src_xyz, wav, rec_xyz, data_out=True):
+        t = self.torch
+        src = np.ascontiguousarray(src_xyz, np.float32).reshape(-1, self.ndim)
+        rec = np.ascontiguousarray(rec_xyz, np.float32).reshape(-1, self.ndim)
+        w = self._dev(wav)
+        assert w.numel() == self.nt * len(src)
+        out = None
+        if data_out is True:
+            out = t.empty((self.nt, len(rec)), dtype=t.float32, device=self.device)
+        elif data_out is not None and data_out is not False:
+            out = data_out
+        _check(self.lib.rtm_forward_probe(self.ctx, len(src), _hp(src), self._ptr(w), len(rec), _hp(rec),
+                                          self._ptr(out), self._stream()))
+        return out
+
+    def adjoint_image(self, rec_xyz, data_in, src_xyz, scale=None, qadj_out=False, image=True, accumulate=False):
+        t = self.torch
+        src = np.ascontiguousarray(src_xyz, np.float32).reshape(-1, self.ndim)
+        rec = np.ascontiguousarray(rec_xyz, np.float32).reshape(-1, self.ndim)
+        din = self._dev(data_in)
+        assert din.numel() == self.nt * len(rec)
+        q = t.empty((self.nt, len(src)), dtype=t.float32, device=self.device) if qadj_out else None
+        img = None
+        if image is True:
+            img = t.zeros(self.n, dtype=t.float32, device=self.device)
+        elif image is not None and image is not False:
+            img = image
+        sc = 1.0 / self.r if scale is None else float(scale)
+        _check(self.lib.rtm_adjoint_image(self.ctx, len(rec), _hp(rec), self._ptr(din), len(src), _hp(src),
+                                          self._ptr(q), sc, 1 if accumulate else 0, self._ptr(img), self._stream()))
+        return img, q
+
+    def offset_gather(self, offsets, scale=None, out=None):
+        t = self.torch
+        offs = np.ascontiguousarray(offsets, np.int32)
+        if out is None:
+            out = t.empty((len(offs),) + self.n, dtype=t.float32, device=self.device)
+        sc = 1.0 / self.r if scale is None else float(scale)
+        _check(self.lib.rtm_offset_gather(self.ctx, len(offs), _hp(offs), sc, self._ptr(out), self._stream()))
+        return out
+
+    def shot_host(self, src_xyz, h_wav, rec_xyz, h_data_in, h_data_out=None, h_image=None, offsets=None,
+                  h_gather=None, scale=None, staging=None):
+        """rtm_shot_host: h_* are pinned CPU torch tensors (or None)."""
+        t = self.torch
+        src = np.ascontiguousarray(src_xyz, np.float32).reshape(-1, self.ndim)
+        rec = np.ascontiguousarray(rec_xyz, np.float32).reshape(-1, self.ndim)
+        nh = 0 if offsets is None else len(offsets)
+        offs = None if offsets is None else np.ascontiguousarray(offsets, np.int32)
+        need = int(self.lib.rtm_shot_staging_bytes(C.byref(self.cfg), len(src), len(rec), nh))
+        if staging is None or staging.numel() < need:
+            staging = t.empty(need, dtype=t.uint8, device=self.device)
+        self._staging = staging
+        sc = 1.0 / self.r if scale is None else float(scale)
+        hp = lambda x: None if x is None else C.c_void_p(x.data_ptr())
+        _check(self.lib.rtm_shot_host(self.ctx, len(src), _hp(src), hp(h_wav), len(rec), _hp(rec), hp(h_data_in),
+                                      hp(h_data_out), sc, hp(h_image), nh, _hp(offs), hp(h_gather),
+                                      C.c_void_p(staging.data_ptr()), staging.numel(), self._stream()))
+        return staging
+
+    def export_probes(self, which):
+        t = self.torch
+        out = t.empty((self.r, self.N), dtype=t.float32, device=self.device)
+        _check(self.lib.rtm_export_probes(self.ctx, int(which), self._ptr(out), self._stream()))
+        return out
+
+    def set_snapshots(self, steps):
+        t = self.torch
+        steps = np.ascontiguousarray(steps, np.int32)
+        nf = 2 if self.physics == 1 else 1
+        out = t.zeros((len(steps), nf, self.Np), dtype=t.float32, device=self.device)
+        _check(self.lib.rtm_set_snapshots(self.ctx, len(steps), _hp(steps), self._ptr(out)))
+        return out
+
+    def export_coeff(self, which):
+        t = self.torch
+        out = t.empty(self.Np, dtype=t.float32, device=self.device)
+        _check(self.lib.rtm_export_coeff(self.ctx, int(which), self._ptr(out), self._stream()))
+        return out
+
+    def launch_count(self) -> int:
+        return int(self.lib.rtm_launch_count(self.ctx))
+
+    def set_option(self, name: str, value: int):
+        _check(self.lib.rtm_set_option(self.ctx, name.encode(), int(value)))

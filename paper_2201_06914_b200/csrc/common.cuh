@@ -1,0 +1,145 @@
+// common.cuh -- layouts, argument blocks and small device helpers shared by the kernels.
+// (CUDA path only; nothing here is used by oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rtm {
+
+// Internal HBM layout.
+//  Fields / coefficient arrays: padded grid P plus a zero halo of H points on every side of every
+//  active axis, z contiguous with pitch pz (multiple of 32 floats); point (jx,jy,jz) of P lives at
+//  org + jx*sx + jy*sy + jz.  H = 4 (acoustic, order-8 star) or 8 (TTI, two chained order-8 first
+//  derivatives).  org, sx, sy are multiples of 4 floats so that z-quads (jz % 4 == 0) are float4-aligned.
+//  Compressed wavefields Uz/Vz: [k][ix][iy][iz] on the PHYSICAL grid only (reading C12), z pitch upz
+//  (multiple of 32), plane stride Nu.  nb % 4 == 0 keeps physical and padded quads aligned.
+struct Layout {
+    int nd;
+    int nx, ny, nz;
+    int Px, Py, Pz;
+    int nb, nby;   // nby = nb in 3D, 0 in 2D (the dummy y axis has no layer)
+    int H, Hy;     // Hy = H in 3D, 0 in 2D
+    int pz;
+    long long sx, sy;
+    long long org;
+    long long fsize;   // floats per field (incl. slack)
+    int upz;
+    long long Nu;      // floats per probe plane
+};
+
+struct InjEntry {
+    int jz;    // padded z index of the grid point
+    int id;    // source / receiver index (column of the value row)
+    float w;   // multilinear corner weight
+    int pad;
+};
+
+// One time step (acoustic: one field; TTI: p and r).
+struct StepArgs {
+    Layout L;
+    const float *u0, *u1;   // current field(s)   (u1: TTI r)
+    float *n0, *n1;         // new field(s)
+    float *d0, *d1;         // increment(s) du = u_cur - u_prev, updated in place
+    const float *K2, *epsh, *delh, *cs, *sn;
+    const float *dampx, *dampy, *dampz;
+    int adjoint;
+    // fused probe: PZ[k][x] += Zrow[k] * new[x]
+    float *PZ;
+    const float *Zrow;
+    int r;
+    // fused injection (row-CSR over (jx,jy) rows, restricted to a bounding box)
+    const int *row_start;
+    const InjEntry *ent;
+    const float *inj_val;   // value row of this step [ninj]
+    float inj_scale;
+    int bx0, bx1, by0, by1, bz0, bz1;
+    // deferred sampling of the CURRENT field (= previous step's result) into smp_out[nsmp]
+    const int *smp_idx;     // [nsmp][nc] offsets from the field base
+    const float *smp_w;     // [nsmp][nc]
+    float *smp_out;         // NULL: nothing to sample in this launch
+    int nsmp, nc;
+    float smp_scale;
+};
+
+// order-8 weights (textbook Fornberg), as the fp32 constants both sides round to (reading C18)
+__device__ __forceinline__ float w2(int j) {
+    return j == 1 ? (float)(8.0 / 5.0) : j == 2 ? (float)(-1.0 / 5.0) : j == 3 ? (float)(8.0 / 315.0) : (float)(-1.0 / 560.0);
+}
+__device__ __forceinline__ float w1(int j) {
+    return j == 1 ? (float)(4.0 / 5.0) : j == 2 ? (float)(-1.0 / 5.0) : j == 3 ? (float)(4.0 / 105.0) : (float)(-1.0 / 280.0);
+}
+
+__device__ __forceinline__ float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+__device__ __forceinline__ void st4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
+// streaming (evict-first) accesses for the probe planes: read once + written once per step
+__device__ __forceinline__ float4 ldcs4(const float *p) { return __ldcs(reinterpret_cast<const float4 *>(p)); }
+__device__ __forceinline__ void stcs4(float *p, float4 v) { __stcs(reinterpret_cast<float4 *>(p), v); }
+
+__device__ __forceinline__ float k1_of(float s) { return s == 0.0f ? 1.0f : (1.0f - s) / (1.0f + s); }
+
+// Deferred receiver sampling: the first ceil(nsmp/nthreads) blocks (linear order) take one point
+// per thread (a4: d[j] = scale * sum_c w_c u[corner]; TTI samples p + r).
+__device__ __forceinline__ void sample_points(const StepArgs &a, int lin_block, int nthreads, int tid) {
+    if (a.smp_out == nullptr) return;
+    long long j = (long long)lin_block * nthreads + tid;
+    if (j >= a.nsmp) return;
+    float acc = 0.0f;
+    for (int c = 0; c < a.nc; c++) {
+        float w = a.smp_w[j * a.nc + c];
+        if (w != 0.0f) {
+            int i = a.smp_idx[j * a.nc + c];
+            float v = a.u0[i];
+            if (a.u1) v += a.u1[i];
+            acc = fmaf(w, v, acc);
+        }
+    }
+    a.smp_out[j] = a.smp_scale * acc;
+}
+
+// Fused injection for one z-quad at row `row` (a3): adds K2 * scale * w * val to the increments.
+__device__ __forceinline__ void inject_quad(const StepArgs &a, long long row, int jz, const float k2[4], float add[4]) {
+    int e0 = a.row_start[row], e1 = a.row_start[row + 1];
+    for (int e = e0; e < e1; e++) {
+        InjEntry en = a.ent[e];
+        int dz = en.jz - jz;
+        if (dz >= 0 && dz < 4) {
+            float v = a.inj_scale * en.w * a.inj_val[en.id];
+#pragma unroll
+            for (int q = 0; q < 4; q++)
+                if (q == dz) add[q] = fmaf(k2[q], v, add[q]);
+        }
+    }
+}
+
+// Fused probe for one z-quad (a5): PZ[k][x] += Z[k] * v for k < r.  p points at plane 0.
+__device__ __forceinline__ void probe_quad(float *p, long long Nu, const float *__restrict__ Zrow, int r, float4 v) {
+    int k = 0;
+    for (; k + 8 <= r; k += 8) {
+        float4 acc[8];
+        float4 za = ldg4(Zrow + k), zb = ldg4(Zrow + k + 4);
+        float z[8] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
+#pragma unroll
+        for (int i = 0; i < 8; i++) acc[i] = ldcs4(p + (long long)(k + i) * Nu);
+#pragma unroll
+        for (int i = 0; i < 8; i++) {
+            acc[i].x = fmaf(z[i], v.x, acc[i].x);
+            acc[i].y = fmaf(z[i], v.y, acc[i].y);
+            acc[i].z = fmaf(z[i], v.z, acc[i].z);
+            acc[i].w = fmaf(z[i], v.w, acc[i].w);
+        }
+#pragma unroll
+        for (int i = 0; i < 8; i++) stcs4(p + (long long)(k + i) * Nu, acc[i]);
+    }
+    for (; k < r; k++) {
+        float z = __ldg(Zrow + k);
+        float4 acc = ldcs4(p + (long long)k * Nu);
+        acc.x = fmaf(z, v.x, acc.x);
+        acc.y = fmaf(z, v.y, acc.y);
+        acc.z = fmaf(z, v.z, acc.z);
+        acc.w = fmaf(z, v.w, acc.w);
+        stcs4(p + (long long)k * Nu, acc);
+    }
+}
+
+}  // namespace rtm

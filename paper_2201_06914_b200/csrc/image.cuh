@@ -1,0 +1,110 @@
+// image.cuh -- image (a7), offset gather (a8), layout conversion and sampling kernels.
+#pragma once
+#include "common.cuh"
+
+namespace rtm {
+
+// a7 (Eq. 3): I[x] (+)= scale * sum_k Uz[k][x] Vz[k][x].  Thread = one physical z-quad.
+__global__ void __launch_bounds__(256) image_kernel(Layout L, const float *__restrict__ U, const float *__restrict__ V,
+                                                    int r, float scale, int accumulate, float *__restrict__ img) {
+    const int nq = L.upz / 4;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long rows = (long long)L.nx * L.ny;
+    if (t >= rows * nq) return;
+    const long long row = t / nq;
+    const int iz = (int)(t % nq) * 4;
+    if (iz >= L.nz) return;
+    const long long o = row * L.upz + iz;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 4
+    for (int k = 0; k < r; k++) {
+        const float4 u = ldcs4(U + k * L.Nu + o), v = ldcs4(V + k * L.Nu + o);
+        acc.x = fmaf(u.x, v.x, acc.x);
+        acc.y = fmaf(u.y, v.y, acc.y);
+        acc.z = fmaf(u.z, v.z, acc.z);
+        acc.w = fmaf(u.w, v.w, acc.w);
+    }
+    const float res[4] = {acc.x, acc.y, acc.z, acc.w};
+    float *out = img + row * L.nz + iz;
+    for (int q = 0; q < 4 && iz + q < L.nz; q++) out[q] = accumulate ? fmaf(scale, res[q], out[q]) : scale * res[q];
+}
+
+// a8 (Eq. 4): G[ih][x] = scale * sum_k Uz[k][x + h e_x] Vz[k][x - h e_x].
+// Thread = one physical z-quad of one row, loops over offsets and probes.  rest = ny * upz / 4 quads
+// per x (x is the slowest axis, so a shift by h is a shift by h * ny * upz floats).
+__global__ void __launch_bounds__(256) gather_kernel(Layout L, const float *__restrict__ U, const float *__restrict__ V,
+                                                     int r, int nh, const int *__restrict__ offs, float scale,
+                                                     float *__restrict__ G) {
+    const int nq = L.upz / 4;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long rows = (long long)L.nx * L.ny;
+    if (t >= rows * nq) return;
+    const long long row = t / nq;
+    const int iz = (int)(t % nq) * 4;
+    if (iz >= L.nz) return;
+    const int ix = (int)(row / L.ny);
+    const long long xs = (long long)L.ny * L.upz;
+    const long long o = row * L.upz + iz;
+    const long long N = rows * L.nz;
+    for (int ih = 0; ih < nh; ih++) {
+        const int h = offs[ih];
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ix + h >= 0 && ix + h < L.nx && ix - h >= 0 && ix - h < L.nx) {
+            const float *pu = U + o + h * xs, *pv = V + o - h * xs;
+#pragma unroll 4
+            for (int k = 0; k < r; k++) {
+                const float4 u = ld4(pu + k * L.Nu), v = ld4(pv + k * L.Nu);
+                acc.x = fmaf(u.x, v.x, acc.x);
+                acc.y = fmaf(u.y, v.y, acc.y);
+                acc.z = fmaf(u.z, v.z, acc.z);
+                acc.w = fmaf(u.w, v.w, acc.w);
+            }
+        }
+        const float res[4] = {acc.x, acc.y, acc.z, acc.w};
+        float *out = G + (long long)ih * N + row * L.nz + iz;
+        for (int q = 0; q < 4 && iz + q < L.nz; q++) out[q] = scale * res[q];
+    }
+}
+
+// canonical [Np] -> internal haloed/pitched layout (halo untouched: it is zeroed once at create)
+__global__ void pack_field_kernel(Layout L, const float *__restrict__ src, float *__restrict__ dst) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long Np = (long long)L.Px * L.Py * L.Pz;
+    if (t >= Np) return;
+    const int jz = (int)(t % L.Pz);
+    const long long q = t / L.Pz;
+    const int jy = (int)(q % L.Py), jx = (int)(q / L.Py);
+    dst[L.org + jx * L.sx + jy * L.sy + jz] = src[t];
+}
+__global__ void unpack_field_kernel(Layout L, const float *__restrict__ src, float *__restrict__ dst) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long Np = (long long)L.Px * L.Py * L.Pz;
+    if (t >= Np) return;
+    const int jz = (int)(t % L.Pz);
+    const long long q = t / L.Pz;
+    const int jy = (int)(q % L.Py), jx = (int)(q / L.Py);
+    dst[t] = src[L.org + jx * L.sx + jy * L.sy + jz];
+}
+// internal probe planes -> canonical [r][N]
+__global__ void unpack_probes_kernel(Layout L, int r, const float *__restrict__ src, float *__restrict__ dst) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long N = (long long)L.nx * L.ny * L.nz;
+    if (t >= N * r) return;
+    const int k = (int)(t / N);
+    const long long x = t % N;
+    const int iz = (int)(x % L.nz);
+    const long long row = x / L.nz;
+    dst[t] = src[k * L.Nu + row * L.upz + iz];
+}
+// Z [nt][r] -> internal [nt][zr] (zr = r rounded up to 8, zero padded) so that rows are float4-aligned
+__global__ void pack_probes_kernel(int nt, int r, int zr, const float *__restrict__ src, float *__restrict__ dst) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)nt * zr) return;
+    const int k = (int)(t % zr);
+    const long long n = t / zr;
+    dst[t] = k < r ? src[n * r + k] : 0.0f;
+}
+// stand-alone sampling of the current field (the last step of a pass has no following step kernel)
+__global__ void __launch_bounds__(256) sample_kernel(const StepArgs a) { sample_points(a, blockIdx.x, 256, threadIdx.x); }
+
+}  // namespace rtm

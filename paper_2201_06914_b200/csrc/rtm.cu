@@ -1,0 +1,683 @@
+// rtm.cu -- host side of the C ABI declared in include/rtm.h: context, workspace carving, geometry
+// tables, time loops, image / gather launches.  All device arithmetic lives in the *.cuh kernels.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/rtm.h"
+#include "acoustic.cuh"
+#include "image.cuh"
+#include "tti.cuh"
+
+using namespace rtm;
+
+static thread_local char g_cuda_err[256] = "";
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                     __FILE__, __LINE__);                                                          \
+            return RTM_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)
+
+static inline long long rup(long long v, long long m) { return (v + m - 1) / m * m; }
+
+// pinned host staging for one set of geometry tables, guarded by an event so that a later call does
+// not overwrite it while an earlier upload is still in flight
+struct HostTables {
+    int *row_start = nullptr;
+    InjEntry *ent = nullptr;
+    int *smp_idx = nullptr;
+    float *smp_w = nullptr;
+    cudaEvent_t done = nullptr;
+    bool pending = false;
+};
+
+struct rtm_ctx {
+    rtm_config cfg;
+    Layout L;
+    char *ws;
+    size_t ws_bytes;
+    int nf;                 // 1 acoustic, 2 TTI
+    float *fld[2][3];       // [field][u_a, u_b, du]
+    float *fields_base;
+    size_t fields_bytes;
+    float *K2, *epsh, *delh, *cs, *sn;
+    float *dampx, *dampy, *dampz;
+    float *Uz, *Vz, *Zf, *Za;
+    int zr;
+    int *row_start;
+    InjEntry *ent;
+    int *smp_idx;
+    float *smp_w;
+    int *offs;
+    long long nrows;
+    bool have_model, have_probes, have_U, have_V;
+    HostTables ht[2];       // [0] forward call, [1] adjoint call
+    int *h_offs;
+    cudaEvent_t offs_done;
+    bool offs_pending;
+    std::vector<int> snap_steps;
+    float *snap_out;
+    long long launches;
+    int opt_graph;
+};
+
+static bool valid_cfg(const rtm_config *c) {
+    if (!c) return false;
+    if (c->ndim != 2 && c->ndim != 3) return false;
+    for (int a = 0; a < c->ndim; a++)
+        if (c->n[a] < 1 || c->n[a] > (1 << 14)) return false;
+    if (!(c->h > 0.f)) return false;
+    if (c->nb < 0 || c->nb % 4 != 0 || c->nb > 1024) return false;
+    if (c->physics != 0 && c->physics != 1) return false;
+    if (c->physics == 1 && c->ndim != 2) return false;
+    if (c->nt < 1 || c->r < 1 || c->r > 256 || c->max_pts < 1) return false;
+    return true;
+}
+
+static void make_layout(const rtm_config *c, Layout *L) {
+    memset(L, 0, sizeof *L);
+    L->nd = c->ndim;
+    L->nx = c->n[0];
+    L->ny = c->ndim == 3 ? c->n[1] : 1;
+    L->nz = c->ndim == 3 ? c->n[2] : c->n[1];
+    L->nb = c->nb;
+    L->nby = c->ndim == 3 ? c->nb : 0;
+    L->H = c->physics == 1 ? 8 : 4;
+    L->Hy = c->ndim == 3 ? L->H : 0;
+    L->Px = L->nx + 2 * c->nb;
+    L->Py = L->ny + 2 * L->nby;
+    L->Pz = L->nz + 2 * c->nb;
+    L->pz = (int)rup(L->Pz + 2 * L->H + 4, 32);
+    L->sy = L->pz;
+    L->sx = (long long)(L->Py + 2 * L->Hy) * L->pz;
+    L->org = (long long)L->H * L->sx + (long long)L->Hy * L->sy + L->H;
+    L->fsize = (long long)(L->Px + 2 * L->H) * L->sx + 64;
+    L->upz = (int)rup(L->nz, 32);
+    L->Nu = (long long)L->nx * L->ny * L->upz;
+}
+
+// workspace carving: returns total bytes; fills pointers when ctx != NULL
+static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        size_t o = off;
+        off += (size_t)rup((long long)bytes, 256);
+        return o;
+    };
+    const int nf = c->physics == 1 ? 2 : 1;
+    const size_t fb = (size_t)L.fsize * 4;
+    size_t o_fields = off;
+    size_t o_f[2][3];
+    for (int f = 0; f < nf; f++)
+        for (int k = 0; k < 3; k++) o_f[f][k] = take(fb);
+    size_t fields_bytes = off - o_fields;
+    size_t o_K2 = take(fb), o_e = 0, o_d = 0, o_c = 0, o_s = 0;
+    if (nf == 2) { o_e = take(fb); o_d = take(fb); o_c = take(fb); o_s = take(fb); }
+    size_t o_dx = take((size_t)(L.Px + 8) * 4), o_dy = take((size_t)(L.Py + 8) * 4), o_dz = take((size_t)(L.Pz + 8) * 4);
+    size_t pb = (size_t)c->r * (size_t)L.Nu * 4;
+    size_t o_U = take(pb), o_V = take(pb);
+    const int zr = (int)rup(c->r, 8);
+    size_t zb = (size_t)c->nt * zr * 4;
+    size_t o_Zf = take(zb), o_Za = take(zb);
+    const long long nrows = (long long)L.Px * L.Py;
+    const int nc = 1 << c->ndim;
+    size_t o_rs = take((size_t)(nrows + 1) * 4);
+    size_t o_en = take((size_t)c->max_pts * nc * sizeof(InjEntry));
+    size_t o_si = take((size_t)c->max_pts * nc * 4), o_sw = take((size_t)c->max_pts * nc * 4);
+    size_t o_of = take(4096 * 4);
+    if (ctx) {
+        char *b = ctx->ws;
+        ctx->nf = nf;
+        for (int f = 0; f < 2; f++)
+            for (int k = 0; k < 3; k++) ctx->fld[f][k] = f < nf ? (float *)(b + o_f[f][k]) : nullptr;
+        ctx->fields_base = (float *)(b + o_fields);
+        ctx->fields_bytes = fields_bytes;
+        ctx->K2 = (float *)(b + o_K2);
+        ctx->epsh = nf == 2 ? (float *)(b + o_e) : nullptr;
+        ctx->delh = nf == 2 ? (float *)(b + o_d) : nullptr;
+        ctx->cs = nf == 2 ? (float *)(b + o_c) : nullptr;
+        ctx->sn = nf == 2 ? (float *)(b + o_s) : nullptr;
+        ctx->dampx = (float *)(b + o_dx);
+        ctx->dampy = (float *)(b + o_dy);
+        ctx->dampz = (float *)(b + o_dz);
+        ctx->Uz = (float *)(b + o_U);
+        ctx->Vz = (float *)(b + o_V);
+        ctx->Zf = (float *)(b + o_Zf);
+        ctx->Za = (float *)(b + o_Za);
+        ctx->zr = zr;
+        ctx->row_start = (int *)(b + o_rs);
+        ctx->ent = (InjEntry *)(b + o_en);
+        ctx->smp_idx = (int *)(b + o_si);
+        ctx->smp_w = (float *)(b + o_sw);
+        ctx->offs = (int *)(b + o_of);
+        ctx->nrows = nrows;
+    }
+    return off;
+}
+
+extern "C" size_t rtm_workspace_bytes(const rtm_config *cfg) {
+    if (!valid_cfg(cfg)) return 0;
+    Layout L;
+    make_layout(cfg, &L);
+    if (L.fsize >= (1LL << 31)) return 0;   // sample tables hold 32-bit offsets
+    return carve(cfg, L, nullptr);
+}
+
+static bool is_device_ptr(const void *p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes, rtm_ctx **out) {
+    if (!out) return RTM_EINVAL;
+    *out = nullptr;
+    size_t need = rtm_workspace_bytes(cfg);
+    if (need == 0 || !d_workspace || ((uintptr_t)d_workspace & 255)) return RTM_EINVAL;
+    if (bytes < need) return RTM_ENOMEM;
+    if (!is_device_ptr(d_workspace)) return RTM_EINVAL;
+    rtm_ctx *c = new (std::nothrow) rtm_ctx();
+    if (!c) return RTM_ENOMEM;
+    c->cfg = *cfg;
+    make_layout(cfg, &c->L);
+    c->ws = (char *)d_workspace;
+    c->ws_bytes = bytes;
+    carve(cfg, c->L, c);
+    c->have_model = c->have_probes = c->have_U = c->have_V = false;
+    c->snap_out = nullptr;
+    c->launches = 0;
+    c->opt_graph = 0;
+    c->offs_pending = false;
+    const int nc = 1 << cfg->ndim;
+    for (int t = 0; t < 2; t++) {
+        HostTables &h = c->ht[t];
+        CU(cudaMallocHost(&h.row_start, (size_t)(c->nrows + 1) * 4));
+        CU(cudaMallocHost(&h.ent, (size_t)cfg->max_pts * nc * sizeof(InjEntry)));
+        CU(cudaMallocHost(&h.smp_idx, (size_t)cfg->max_pts * nc * 4));
+        CU(cudaMallocHost(&h.smp_w, (size_t)cfg->max_pts * nc * 4));
+        CU(cudaEventCreateWithFlags(&h.done, cudaEventDisableTiming));
+    }
+    CU(cudaMallocHost(&c->h_offs, 4096 * 4));
+    CU(cudaEventCreateWithFlags(&c->offs_done, cudaEventDisableTiming));
+    *out = c;
+    return RTM_OK;
+}
+
+extern "C" void rtm_destroy(rtm_ctx *c) {
+    if (!c) return;
+    for (int t = 0; t < 2; t++) {
+        HostTables &h = c->ht[t];
+        if (h.done) { cudaEventSynchronize(h.done); cudaEventDestroy(h.done); }
+        cudaFreeHost(h.row_start); cudaFreeHost(h.ent); cudaFreeHost(h.smp_idx); cudaFreeHost(h.smp_w);
+    }
+    if (c->offs_done) { cudaEventSynchronize(c->offs_done); cudaEventDestroy(c->offs_done); }
+    cudaFreeHost(c->h_offs);
+    delete c;
+}
+
+// ---- O1: coefficients on the host (fp64, one rounding to fp32) ---------------------------------
+extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
+                               const float *h_theta, float *h_K2, float *h_epsh, float *h_delh, float *h_cos,
+                               float *h_sin, float *h_damp1d) {
+    if (!valid_cfg(cfg) || !h_vp || !h_K2 || !h_damp1d) return RTM_EINVAL;
+    const bool tti = cfg->physics == 1;
+    if (tti && (!h_eps || !h_delta || !h_theta || !h_epsh || !h_delh || !h_cos || !h_sin)) return RTM_EINVAL;
+    Layout L;
+    make_layout(cfg, &L);
+    const long long N = (long long)L.nx * L.ny * L.nz;
+    const double h = (double)cfg->h, dt = cfg->dt;
+    const int nb = cfg->nb;
+    double vmax = 0.0;
+    for (long long i = 0; i < N; i++) vmax = std::max(vmax, (double)h_vp[i]);
+    const double sigma_max = nb > 0 ? vmax * std::log(1000.0) / ((double)nb * h) : 0.0;
+    // per-axis profiles sigma_a(i) dt; the dummy y axis of a 2D grid contributes nothing
+    const int P[3] = {L.Px, L.Py, L.Pz};
+    const int lay[3] = {nb, L.nby, nb};
+    std::vector<double> prof[3];
+    float *tab = h_damp1d;
+    for (int a = 0; a < 3; a++) {
+        prof[a].assign(P[a], 0.0);
+        if (cfg->ndim == 2 && a == 1) continue;
+        for (int i = 0; i < P[a]; i++) {
+            const int depth = std::max(0, std::max(nb - i, i - (P[a] - 1 - nb)));
+            const double s = nb > 0 ? (double)depth / (double)nb : 0.0;
+            const double phi = s - std::sin(2.0 * M_PI * s) / (2.0 * M_PI);
+            prof[a][i] = sigma_max * phi * dt;
+            tab[i] = (float)prof[a][i];
+        }
+        tab += P[a];
+    }
+    const int nn[3] = {L.nx, L.ny, L.nz};
+    for (int jx = 0; jx < L.Px; jx++)
+        for (int jy = 0; jy < L.Py; jy++)
+            for (int jz = 0; jz < L.Pz; jz++) {
+                const int ix = std::min(std::max(jx - lay[0], 0), nn[0] - 1);
+                const int iy = std::min(std::max(jy - lay[1], 0), nn[1] - 1);
+                const int iz = std::min(std::max(jz - lay[2], 0), nn[2] - 1);
+                const long long s = ((long long)ix * L.ny + iy) * L.nz + iz;
+                const long long d = ((long long)jx * L.Py + jy) * L.Pz + jz;
+                const double c = h_vp[s];
+                const double sdt = prof[0][jx] + prof[1][jy] + prof[2][jz];
+                h_K2[d] = (float)(c * c * dt * dt / (h * h * (1.0 + sdt)));
+                if (tti) {
+                    const double e = h_eps[s];
+                    const double dl = std::min((double)h_delta[s], e);
+                    const double th = h_theta[s];
+                    h_epsh[d] = (float)(1.0 + 2.0 * e);
+                    h_delh[d] = (float)std::sqrt(1.0 + 2.0 * dl);
+                    h_cos[d] = (float)std::cos(th);
+                    h_sin[d] = (float)std::sin(th);
+                }
+            }
+    return RTM_OK;
+}
+
+static int launch_pack(rtm_ctx *c, const float *src, float *dst, cudaStream_t st) {
+    const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pz;
+    pack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, st>>>(c->L, src, dst);
+    c->launches++;
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
+extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh, const float *d_delh,
+                             const float *d_cos, const float *d_sin, const float *h_damp1d, void *stream) {
+    if (!c || !d_K2 || !h_damp1d) return RTM_EINVAL;
+    const bool tti = c->cfg.physics == 1;
+    if (tti && (!d_epsh || !d_delh || !d_cos || !d_sin)) return RTM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Layout &L = c->L;
+    // zero everything up to the probe planes once (halo of fields and coefficients stays zero)
+    CU(cudaMemsetAsync(c->ws, 0, (size_t)((char *)c->Uz - c->ws), st));
+    int rc;
+    if ((rc = launch_pack(c, d_K2, c->K2, st))) return rc;
+    if (tti) {
+        if ((rc = launch_pack(c, d_epsh, c->epsh, st))) return rc;
+        if ((rc = launch_pack(c, d_delh, c->delh, st))) return rc;
+        if ((rc = launch_pack(c, d_cos, c->cs, st))) return rc;
+        if ((rc = launch_pack(c, d_sin, c->sn, st))) return rc;
+    }
+    // small tables: pageable source, the copy is staged before the call returns
+    const float *t = h_damp1d;
+    CU(cudaMemcpyAsync(c->dampx, t, (size_t)L.Px * 4, cudaMemcpyHostToDevice, st));
+    t += L.Px;
+    if (c->cfg.ndim == 3) {
+        CU(cudaMemcpyAsync(c->dampy, t, (size_t)L.Py * 4, cudaMemcpyHostToDevice, st));
+        t += L.Py;
+    }
+    CU(cudaMemcpyAsync(c->dampz, t, (size_t)L.Pz * 4, cudaMemcpyHostToDevice, st));
+    c->have_model = true;
+    c->have_U = c->have_V = false;
+    return RTM_OK;
+}
+
+extern "C" int rtm_set_probes(rtm_ctx *c, const float *d_Zf, const float *d_Za, void *stream) {
+    if (!c || !d_Zf || !d_Za) return RTM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long tot = (long long)c->cfg.nt * c->zr;
+    pack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(c->cfg.nt, c->cfg.r, c->zr, d_Zf, c->Zf);
+    pack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(c->cfg.nt, c->cfg.r, c->zr, d_Za, c->Za);
+    c->launches += 2;
+    CU(cudaGetLastError());
+    c->have_probes = true;
+    return RTM_OK;
+}
+
+// ---- geometry (reading C9): multilinear corners and weights -------------------------------------
+struct Corner { int jx, jy, jz; float w; };
+
+// returns the number of corners (2^d) or -1 if the position is outside [0,(n_a-1)h]
+static int corners_of(const rtm_config &cfg, const Layout &L, const float *xyz, Corner *out) {
+    const int nn[3] = {L.nx, L.ny, L.nz};
+    int base[3] = {0, 0, 0};
+    double frac[3] = {0.0, 0.0, 0.0};
+    int k = 0;
+    for (int a = 0; a < 3; a++) {
+        if (cfg.ndim == 2 && a == 1) continue;
+        const double f = (double)xyz[k++] / (double)cfg.h;
+        if (!(f >= 0.0) || f > (double)(nn[a] - 1)) return -1;
+        int i = (int)std::floor(f);
+        i = std::max(0, std::min(i, nn[a] - 2));
+        base[a] = i;
+        frac[a] = f - (double)i;
+    }
+    int cnt = 0;
+    for (int bx = 0; bx < 2; bx++)
+        for (int by = 0; by < 2; by++)
+            for (int bz = 0; bz < 2; bz++) {
+                if (cfg.ndim == 2 && by) continue;
+                Corner &co = out[cnt++];
+                if ((bx && nn[0] == 1) || (by && nn[1] == 1) || (bz && nn[2] == 1)) { co = {0, 0, 0, 0.f}; continue; }
+                double w = bx ? frac[0] : 1.0 - frac[0];
+                if (cfg.ndim == 3) w *= by ? frac[1] : 1.0 - frac[1];
+                w *= bz ? frac[2] : 1.0 - frac[2];
+                co.jx = base[0] + bx + L.nb;
+                co.jy = base[1] + by + L.nby;
+                co.jz = base[2] + bz + L.nb;
+                co.w = (float)w;
+            }
+    return cnt;
+}
+
+struct PassGeom {
+    int ninj, nsmp, nc;
+    int bx0, bx1, by0, by1, bz0, bz1;
+};
+
+// Build injection (row-CSR) and sampling tables on the host and upload them.
+static int build_geometry(rtm_ctx *c, int slot, int ninj, const float *inj_xyz, int nsmp, const float *smp_xyz,
+                          PassGeom *g, cudaStream_t st) {
+    const rtm_config &cfg = c->cfg;
+    const Layout &L = c->L;
+    const int nd = cfg.ndim, nc = 1 << nd;
+    HostTables &h = c->ht[slot];
+    if (h.pending) { CU(cudaEventSynchronize(h.done)); h.pending = false; }
+    g->ninj = ninj; g->nsmp = nsmp; g->nc = nc;
+    g->bx0 = g->by0 = g->bz0 = 1 << 30;
+    g->bx1 = g->by1 = g->bz1 = -1;
+    struct Tmp { long long row; int jz, id; float w; };
+    std::vector<Tmp> tmp;
+    tmp.reserve((size_t)ninj * nc);
+    Corner co[8];
+    for (int s = 0; s < ninj; s++) {
+        if (corners_of(cfg, L, inj_xyz + (size_t)s * nd, co) < 0) return RTM_EINVAL;
+        for (int k = 0; k < nc; k++) {
+            if (co[k].w == 0.f) continue;
+            tmp.push_back({(long long)co[k].jx * L.Py + co[k].jy, co[k].jz, s, co[k].w});
+            g->bx0 = std::min(g->bx0, co[k].jx); g->bx1 = std::max(g->bx1, co[k].jx);
+            g->by0 = std::min(g->by0, co[k].jy); g->by1 = std::max(g->by1, co[k].jy);
+            g->bz0 = std::min(g->bz0, co[k].jz); g->bz1 = std::max(g->bz1, co[k].jz);
+        }
+    }
+    std::sort(tmp.begin(), tmp.end(), [](const Tmp &a, const Tmp &b) {
+        if (a.row != b.row) return a.row < b.row;
+        if (a.jz != b.jz) return a.jz < b.jz;
+        return a.id < b.id;
+    });
+    std::fill(h.row_start, h.row_start + c->nrows + 1, 0);
+    for (const Tmp &t : tmp) h.row_start[t.row + 1]++;
+    for (long long i = 0; i < c->nrows; i++) h.row_start[i + 1] += h.row_start[i];
+    for (size_t i = 0; i < tmp.size(); i++) h.ent[i] = {tmp[i].jz, tmp[i].id, tmp[i].w, 0};
+    for (int s = 0; s < nsmp; s++) {
+        if (corners_of(cfg, L, smp_xyz + (size_t)s * nd, co) < 0) return RTM_EINVAL;
+        for (int k = 0; k < nc; k++) {
+            h.smp_idx[(size_t)s * nc + k] = (int)(L.org + co[k].jx * L.sx + co[k].jy * L.sy + co[k].jz);
+            h.smp_w[(size_t)s * nc + k] = co[k].w;
+        }
+    }
+    CU(cudaMemcpyAsync(c->row_start, h.row_start, (size_t)(c->nrows + 1) * 4, cudaMemcpyHostToDevice, st));
+    if (!tmp.empty())
+        CU(cudaMemcpyAsync(c->ent, h.ent, tmp.size() * sizeof(InjEntry), cudaMemcpyHostToDevice, st));
+    if (nsmp > 0) {
+        CU(cudaMemcpyAsync(c->smp_idx, h.smp_idx, (size_t)nsmp * nc * 4, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(c->smp_w, h.smp_w, (size_t)nsmp * nc * 4, cudaMemcpyHostToDevice, st));
+    }
+    CU(cudaEventRecord(h.done, st));
+    h.pending = true;
+    return RTM_OK;
+}
+
+// ---- one propagation pass (a1-a6) ---------------------------------------------------------------
+static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
+    const Layout &L = c->L;
+    if (c->cfg.physics == 1) {
+        *grid = dim3((L.Pz + TTI_TZ - 1) / TTI_TZ, (L.Px + TTI_TX - 1) / TTI_TX, 1);
+        *block = dim3(16, 16, 1);
+        *smem = TTI_SMEM;
+    } else if (c->cfg.ndim == 2) {
+        *grid = dim3((L.Pz + 127) / 128, (L.Px + 7) / 8, 1);
+        *block = dim3(32, 8, 1);
+        *smem = 0;
+    } else {
+        *grid = dim3((L.Pz + 127) / 128, (L.Py + 7) / 8, L.Px);
+        *block = dim3(32, 8, 1);
+        *smem = 0;
+    }
+}
+
+static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+    if (c->cfg.physics == 1) tti_step_kernel<<<grid, block, smem, st>>>(a);
+    else if (c->cfg.ndim == 2) acoustic_step_kernel<2><<<grid, block, 0, st>>>(a);
+    else acoustic_step_kernel<3><<<grid, block, 0, st>>>(a);
+    c->launches++;
+    return RTM_OK;
+}
+
+static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_inj_val, float *d_smp_out,
+                    float *PZ, const float *Z, cudaStream_t st) {
+    const rtm_config &cfg = c->cfg;
+    const Layout &L = c->L;
+    const int nt = cfg.nt, d = cfg.ndim;
+    CU(cudaMemsetAsync(c->fields_base, 0, c->fields_bytes, st));
+    CU(cudaMemsetAsync(PZ, 0, (size_t)cfg.r * (size_t)L.Nu * 4, st));
+
+    StepArgs a;
+    memset(&a, 0, sizeof a);
+    a.L = L;
+    a.K2 = c->K2; a.epsh = c->epsh; a.delh = c->delh; a.cs = c->cs; a.sn = c->sn;
+    a.dampx = c->dampx; a.dampy = c->dampy; a.dampz = c->dampz;
+    a.adjoint = adjoint;
+    a.PZ = PZ;
+    a.r = cfg.r;
+    a.row_start = c->row_start;
+    a.ent = c->ent;
+    double inj_scale = adjoint ? (double)cfg.h * (double)cfg.h : std::pow((double)cfg.h, 2.0 - d);
+    double smp_scale = adjoint ? std::pow((double)cfg.h, -(double)d) : 1.0;
+    if (cfg.physics == 1) { if (adjoint) inj_scale *= 0.5; else smp_scale *= 0.5; }
+    a.inj_scale = (float)inj_scale;
+    a.smp_scale = (float)smp_scale;
+    a.bx0 = g.bx0; a.bx1 = g.bx1; a.by0 = g.by0; a.by1 = g.by1; a.bz0 = g.bz0; a.bz1 = g.bz1;
+    a.smp_idx = c->smp_idx;
+    a.smp_w = c->smp_w;
+    a.nsmp = g.nsmp;
+    a.nc = g.nc;
+
+    dim3 grid, block;
+    size_t smem;
+    step_grid(c, &grid, &block, &smem);
+    const long long nblocks = (long long)grid.x * grid.y * grid.z;
+    const bool want_smp = d_smp_out != nullptr && g.nsmp > 0;
+    const bool deferred = want_smp && (long long)g.nsmp <= nblocks * 256;
+    const unsigned smp_blocks = (unsigned)((g.nsmp + 255) / 256);
+
+    int cur = 0;
+    const long long Np = (long long)L.Px * L.Py * L.Pz;
+    for (int step = 0; step < nt; step++) {
+        const int n = adjoint ? nt - 1 - step : step;
+        const int nprev = adjoint ? n + 1 : n - 1;
+        a.u0 = c->fld[0][cur]; a.n0 = c->fld[0][cur ^ 1]; a.d0 = c->fld[0][2];
+        a.u1 = c->fld[1][cur]; a.n1 = c->fld[1][cur ^ 1]; a.d1 = c->fld[1][2];
+        a.Zrow = Z + (size_t)n * c->zr;
+        a.inj_val = d_inj_val + (size_t)n * g.ninj;
+        a.smp_out = (deferred && step > 0) ? d_smp_out + (size_t)nprev * g.nsmp : nullptr;
+        launch_step(c, a, grid, block, smem, st);
+        cur ^= 1;
+        if (want_smp && (!deferred || step == nt - 1)) {
+            StepArgs s = a;   // sample the field just computed
+            s.u0 = c->fld[0][cur]; s.u1 = c->fld[1][cur];
+            s.smp_out = d_smp_out + (size_t)n * g.nsmp;
+            sample_kernel<<<smp_blocks, 256, 0, st>>>(s);
+            c->launches++;
+        }
+        for (size_t q = 0; q < c->snap_steps.size(); q++)
+            if (c->snap_steps[q] == n && c->snap_out)
+                for (int f = 0; f < c->nf; f++) {
+                    unpack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, st>>>(
+                        L, c->fld[f][cur], c->snap_out + ((long long)q * c->nf + f) * Np);
+                    c->launches++;
+                }
+    }
+    CU(cudaGetLastError());
+    c->snap_steps.clear();
+    c->snap_out = nullptr;
+    return RTM_OK;
+}
+
+extern "C" int rtm_forward_probe(rtm_ctx *c, int nsrc, const float *h_src_xyz, const float *d_wav, int nrec,
+                                 const float *h_rec_xyz, float *d_data_out, void *stream) {
+    if (!c || nsrc < 1 || !h_src_xyz || !d_wav || nrec < 0 || (nrec > 0 && !h_rec_xyz)) return RTM_EINVAL;
+    if (nsrc > c->cfg.max_pts || nrec > c->cfg.max_pts) return RTM_EINVAL;
+    if (!c->have_model || !c->have_probes) return RTM_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    PassGeom g;
+    int rc = build_geometry(c, 0, nsrc, h_src_xyz, nrec, h_rec_xyz, &g, st);
+    if (rc) return rc;
+    c->have_U = false;
+    rc = run_pass(c, 0, g, d_wav, d_data_out, c->Uz, c->Zf, st);
+    if (rc) return rc;
+    c->have_U = true;
+    c->have_V = false;
+    return RTM_OK;
+}
+
+static int launch_image(rtm_ctx *c, float scale, int accumulate, float *d_image, cudaStream_t st) {
+    const Layout &L = c->L;
+    const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
+    image_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, scale, accumulate, d_image);
+    c->launches++;
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
+extern "C" int rtm_adjoint_image(rtm_ctx *c, int nrec, const float *h_rec_xyz, const float *d_data_in, int nsrc,
+                                 const float *h_src_xyz, float *d_qadj_out, float scale, int accumulate,
+                                 float *d_image, void *stream) {
+    if (!c || nrec < 1 || !h_rec_xyz || !d_data_in || nsrc < 0 || (nsrc > 0 && !h_src_xyz)) return RTM_EINVAL;
+    if (nsrc > c->cfg.max_pts || nrec > c->cfg.max_pts) return RTM_EINVAL;
+    if (!c->have_model || !c->have_probes) return RTM_ESTATE;
+    if (d_image && !c->have_U) return RTM_ESTATE;   // adjoint before forward
+    cudaStream_t st = (cudaStream_t)stream;
+    PassGeom g;
+    int rc = build_geometry(c, 1, nrec, h_rec_xyz, nsrc, h_src_xyz, &g, st);
+    if (rc) return rc;
+    c->have_V = false;
+    rc = run_pass(c, 1, g, d_data_in, d_qadj_out, c->Vz, c->Za, st);
+    if (rc) return rc;
+    c->have_V = true;
+    if (d_image) return launch_image(c, scale, accumulate, d_image, st);
+    return RTM_OK;
+}
+
+extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float scale, float *d_gather, void *stream) {
+    if (!c || nh < 1 || nh > 4096 || !h_offsets || !d_gather) return RTM_EINVAL;
+    if (!c->have_U || !c->have_V) return RTM_ESTATE;
+    for (int i = 0; i < nh; i++)
+        if (std::abs(h_offsets[i]) >= c->cfg.n[0]) return RTM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (c->offs_pending) { CU(cudaEventSynchronize(c->offs_done)); c->offs_pending = false; }
+    memcpy(c->h_offs, h_offsets, (size_t)nh * 4);
+    CU(cudaMemcpyAsync(c->offs, c->h_offs, (size_t)nh * 4, cudaMemcpyHostToDevice, st));
+    CU(cudaEventRecord(c->offs_done, st));
+    c->offs_pending = true;
+    const Layout &L = c->L;
+    const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
+    gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, c->offs, scale, d_gather);
+    c->launches++;
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
+extern "C" size_t rtm_shot_staging_bytes(const rtm_config *cfg, int nsrc, int nrec, int nh) {
+    if (!valid_cfg(cfg) || nsrc < 1 || nrec < 1 || nh < 0) return 0;
+    Layout L;
+    make_layout(cfg, &L);
+    const size_t N = (size_t)L.nx * L.ny * L.nz, nt = (size_t)cfg->nt;
+    size_t b = 0;
+    b += (size_t)rup((long long)(nt * nsrc * 4), 256);
+    b += 2 * (size_t)rup((long long)(nt * nrec * 4), 256);
+    b += (size_t)rup((long long)(N * 4), 256);
+    b += (size_t)rup((long long)((size_t)nh * N * 4), 256);
+    return b + 256;
+}
+
+extern "C" int rtm_shot_host(rtm_ctx *c, int nsrc, const float *h_src_xyz, const float *h_wav, int nrec,
+                             const float *h_rec_xyz, const float *h_data_in, float *h_data_out, float scale,
+                             float *h_image, int nh, const int *h_offsets, float *h_gather, void *d_staging,
+                             size_t staging_bytes, void *stream) {
+    if (!c || !h_wav || !h_data_in || !d_staging) return RTM_EINVAL;
+    size_t need = rtm_shot_staging_bytes(&c->cfg, nsrc, nrec, nh);
+    if (need == 0 || ((uintptr_t)d_staging & 255)) return RTM_EINVAL;
+    if (staging_bytes < need) return RTM_ENOMEM;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Layout &L = c->L;
+    const size_t N = (size_t)L.nx * L.ny * L.nz, nt = (size_t)c->cfg.nt;
+    char *p = (char *)d_staging;
+    float *d_wav = (float *)p;  p += rup((long long)(nt * nsrc * 4), 256);
+    float *d_din = (float *)p;  p += rup((long long)(nt * nrec * 4), 256);
+    float *d_dout = (float *)p; p += rup((long long)(nt * nrec * 4), 256);
+    float *d_img = (float *)p;  p += rup((long long)(N * 4), 256);
+    float *d_gat = (float *)p;
+    CU(cudaMemcpyAsync(d_wav, h_wav, nt * nsrc * 4, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d_din, h_data_in, nt * nrec * 4, cudaMemcpyHostToDevice, st));
+    int rc = rtm_forward_probe(c, nsrc, h_src_xyz, d_wav, nrec, h_rec_xyz, h_data_out ? d_dout : nullptr, stream);
+    if (rc) return rc;
+    if (h_data_out) CU(cudaMemcpyAsync(h_data_out, d_dout, nt * nrec * 4, cudaMemcpyDeviceToHost, st));
+    rc = rtm_adjoint_image(c, nrec, h_rec_xyz, d_din, nsrc, h_src_xyz, nullptr, scale, 0, h_image ? d_img : nullptr, stream);
+    if (rc) return rc;
+    if (h_image) CU(cudaMemcpyAsync(h_image, d_img, N * 4, cudaMemcpyDeviceToHost, st));
+    if (nh > 0 && h_gather) {
+        rc = rtm_offset_gather(c, nh, h_offsets, scale, d_gat, stream);
+        if (rc) return rc;
+        CU(cudaMemcpyAsync(h_gather, d_gat, (size_t)nh * N * 4, cudaMemcpyDeviceToHost, st));
+    }
+    return RTM_OK;
+}
+
+// ---- test hooks ----------------------------------------------------------------------------------
+extern "C" int rtm_export_probes(rtm_ctx *c, int which, float *d_out, void *stream) {
+    if (!c || !d_out || (which != 0 && which != 1)) return RTM_EINVAL;
+    if (which == 0 ? !c->have_U : !c->have_V) return RTM_ESTATE;
+    const Layout &L = c->L;
+    const long long tot = (long long)L.nx * L.ny * L.nz * c->cfg.r;
+    unpack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(L, c->cfg.r, which ? c->Vz : c->Uz, d_out);
+    c->launches++;
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
+extern "C" int rtm_set_snapshots(rtm_ctx *c, int nsnap, const int *h_steps, float *d_out) {
+    if (!c || nsnap < 0 || (nsnap > 0 && (!h_steps || !d_out))) return RTM_EINVAL;
+    c->snap_steps.assign(h_steps, h_steps + nsnap);
+    c->snap_out = nsnap ? d_out : nullptr;
+    return RTM_OK;
+}
+
+extern "C" int rtm_export_coeff(rtm_ctx *c, int which, float *d_out, void *stream) {
+    if (!c || !d_out || which < 0 || which > 4) return RTM_EINVAL;
+    if (!c->have_model) return RTM_ESTATE;
+    const float *src[5] = {c->K2, c->epsh, c->delh, c->cs, c->sn};
+    if (!src[which]) return RTM_EINVAL;
+    const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pz;
+    unpack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c->L, src[which], d_out);
+    c->launches++;
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
+extern "C" long long rtm_launch_count(const rtm_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
+    if (!c || !name) return RTM_EINVAL;
+    if (!strcmp(name, "graph")) { c->opt_graph = value; return RTM_OK; }
+    return RTM_EINVAL;
+}
+
+extern "C" const char *rtm_strerror(int code) {
+    switch (code) {
+        case RTM_OK: return "ok";
+        case RTM_EINVAL: return "invalid argument";
+        case RTM_ENOMEM: return "workspace too small";
+        case RTM_ECUDA: return "CUDA error";
+        case RTM_ESTATE: return "call out of order";
+        default: return "unknown error";
+    }
+}
+extern "C" const char *rtm_last_cuda_error(void) { return g_cuda_err; }

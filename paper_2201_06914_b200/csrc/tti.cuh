@@ -1,0 +1,164 @@
+// tti.cuh -- 2D pseudo-acoustic TTI time step (a2) with fused damping, injection, deferred sampling
+// and probe accumulation of the single field (p + r)/2 (reading C10).
+//
+//   forward (post-mix, O5):  A = H_perp p, B = H_par r,
+//        dp_new = K1 dp + K2 (epsh A + delh B),  dr_new = K1 dr + K2 (delh A + B)
+//   adjoint (pre-mix, O6):   a = epsh p + delh r, b = delh p + r, A = H_perp a, B = H_par b,
+//        dp_new = K1 dp + K2 A,                  dr_new = K1 dr + K2 B
+//   H_perp f = Dx(cos g) - Dz(sin g), g = cos Dx f - sin Dz f ;  H_par f = Dx(sin g) + Dz(cos g),
+//   g = sin Dx f + cos Dz f ; D = undivided centred order-8 first derivative; g is zero outside P
+//   (cos = sin = 0 in the coefficient halo does that).
+//
+// Two-stage tile kernel: stage 1 loads the (mixed) fields with a halo of 8 into shared memory,
+// stage 2 forms the four products cos g_perp, sin g_perp, sin g_par, cos g_par on the tile + halo 4,
+// stage 3 differentiates them.  Tile = 16 (x) x 64 (z), 256 threads, one z-quad per thread.
+#pragma once
+#include "common.cuh"
+
+namespace rtm {
+
+constexpr int TTI_TX = 16, TTI_TZ = 64;
+constexpr int TTI_FX = TTI_TX + 16, TTI_FZ = TTI_TZ + 16;   // field tile (halo 8)
+constexpr int TTI_GX = TTI_TX + 8, TTI_GZ = TTI_TZ + 8;     // product tile (halo 4)
+constexpr int TTI_SMEM = (2 * TTI_FX * TTI_FZ + 4 * TTI_GX * TTI_GZ) * 4;
+
+__global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    float *sA = smem;                          // [FX][FZ]
+    float *sB = sA + TTI_FX * TTI_FZ;
+    float *P1 = sB + TTI_FX * TTI_FZ;          // cos g_perp  [GX][GZ]
+    float *P2 = P1 + TTI_GX * TTI_GZ;          // sin g_perp
+    float *P3 = P2 + TTI_GX * TTI_GZ;          // sin g_par
+    float *P4 = P3 + TTI_GX * TTI_GZ;          // cos g_par
+
+    const Layout &L = a.L;
+    const int tid = threadIdx.y * 16 + threadIdx.x;
+    const int lin_block = blockIdx.y * gridDim.x + blockIdx.x;
+    sample_points(a, lin_block, 256, tid);
+
+    const int z0 = blockIdx.x * TTI_TZ, x0 = blockIdx.y * TTI_TX;
+
+    // ---- stage 1: (mixed) fields, halo 8 ----
+    for (int i = tid; i < TTI_FX * (TTI_FZ / 4); i += 256) {
+        const int lx = i / (TTI_FZ / 4), lq = i % (TTI_FZ / 4);
+        const int jx = x0 - 8 + lx, jz = z0 - 8 + lq * 4;
+        float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;
+        if (jx < L.Px + 8 && jz + 3 < L.pz - 8) {
+            const long long o = L.org + jx * L.sx + jz;
+            va = ld4(a.u0 + o);
+            vb = ld4(a.u1 + o);
+            if (a.adjoint) {
+                const float4 e = ld4(a.epsh + o), d = ld4(a.delh + o);
+                float4 ma, mb;
+                ma.x = fmaf(e.x, va.x, d.x * vb.x); mb.x = fmaf(d.x, va.x, vb.x);
+                ma.y = fmaf(e.y, va.y, d.y * vb.y); mb.y = fmaf(d.y, va.y, vb.y);
+                ma.z = fmaf(e.z, va.z, d.z * vb.z); mb.z = fmaf(d.z, va.z, vb.z);
+                ma.w = fmaf(e.w, va.w, d.w * vb.w); mb.w = fmaf(d.w, va.w, vb.w);
+                va = ma; vb = mb;
+            }
+        }
+        st4(sA + lx * TTI_FZ + lq * 4, va);
+        st4(sB + lx * TTI_FZ + lq * 4, vb);
+    }
+    __syncthreads();
+
+    // ---- stage 2: rotated gradients times cos / sin, halo 4 ----
+    for (int i = tid; i < TTI_GX * TTI_GZ; i += 256) {
+        const int lx = i / TTI_GZ, lz = i % TTI_GZ;
+        const int jx = x0 - 4 + lx, jz = z0 - 4 + lz;
+        float cs = 0.f, sn = 0.f;
+        if (jx < L.Px + 8 && jz < L.pz - 8) {
+            const long long o = L.org + jx * L.sx + jz;
+            cs = a.cs[o];
+            sn = a.sn[o];
+        }
+        const float *fa = sA + (lx + 4) * TTI_FZ + (lz + 4);
+        const float *fb = sB + (lx + 4) * TTI_FZ + (lz + 4);
+        float ax = 0.f, az = 0.f, bx = 0.f, bz = 0.f;
+#pragma unroll
+        for (int j = 4; j >= 1; j--) {
+            const float w = w1(j);
+            ax = fmaf(w, fa[j * TTI_FZ] - fa[-j * TTI_FZ], ax);
+            az = fmaf(w, fa[j] - fa[-j], az);
+            bx = fmaf(w, fb[j * TTI_FZ] - fb[-j * TTI_FZ], bx);
+            bz = fmaf(w, fb[j] - fb[-j], bz);
+        }
+        const float gp = cs * ax - sn * az;   // g_perp
+        const float gl = sn * bx + cs * bz;   // g_par
+        P1[i] = cs * gp;
+        P2[i] = sn * gp;
+        P3[i] = sn * gl;
+        P4[i] = cs * gl;
+    }
+    __syncthreads();
+
+    // ---- stage 3: second derivative pass, update, inject, probe ----
+    const int lx = threadIdx.y, lz = threadIdx.x * 4;
+    const int jx = x0 + lx, jz = z0 + lz;
+    if (jx >= L.Px || jz >= L.Pz) return;
+    const long long off = L.org + jx * L.sx + jz;
+
+    float A[4], B[4];
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        const int g = (lx + 4) * TTI_GZ + (lz + q + 4);
+        float dx1 = 0.f, dz2 = 0.f, dx3 = 0.f, dz4 = 0.f;
+#pragma unroll
+        for (int j = 4; j >= 1; j--) {
+            const float w = w1(j);
+            dx1 = fmaf(w, P1[g + j * TTI_GZ] - P1[g - j * TTI_GZ], dx1);
+            dz2 = fmaf(w, P2[g + j] - P2[g - j], dz2);
+            dx3 = fmaf(w, P3[g + j * TTI_GZ] - P3[g - j * TTI_GZ], dx3);
+            dz4 = fmaf(w, P4[g + j] - P4[g - j], dz4);
+        }
+        A[q] = dx1 - dz2;
+        B[q] = dx3 + dz4;
+    }
+
+    const float4 p4 = ld4(a.u0 + off), r4 = ld4(a.u1 + off);
+    const float4 dp4 = ld4(a.d0 + off), dr4 = ld4(a.d1 + off);
+    const float4 k24 = ld4(a.K2 + off);
+    const float pc[4] = {p4.x, p4.y, p4.z, p4.w}, rc[4] = {r4.x, r4.y, r4.z, r4.w};
+    const float dp[4] = {dp4.x, dp4.y, dp4.z, dp4.w}, dr[4] = {dr4.x, dr4.y, dr4.z, dr4.w};
+    const float k2[4] = {k24.x, k24.y, k24.z, k24.w};
+    float eh[4] = {1.f, 1.f, 1.f, 1.f}, dh[4] = {0.f, 0.f, 0.f, 0.f};
+    if (!a.adjoint) {
+        const float4 e4 = ld4(a.epsh + off), d4 = ld4(a.delh + off);
+        eh[0] = e4.x; eh[1] = e4.y; eh[2] = e4.z; eh[3] = e4.w;
+        dh[0] = d4.x; dh[1] = d4.y; dh[2] = d4.z; dh[3] = d4.w;
+    }
+    const float sx = a.dampx[jx];
+    const float4 dz4 = ld4(a.dampz + jz);
+    const float dzv[4] = {dz4.x, dz4.y, dz4.z, dz4.w};
+
+    float inj[4] = {0.f, 0.f, 0.f, 0.f};
+    if (jx >= a.bx0 && jx <= a.bx1 && jz + 3 >= a.bz0 && jz <= a.bz1) inject_quad(a, jx, jz, k2, inj);
+
+    float pn[4], rn[4], dpn[4], drn[4], pr[4];
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        const float k1 = k1_of(sx + dzv[q]);
+        const float ra = a.adjoint ? A[q] : fmaf(eh[q], A[q], dh[q] * B[q]);
+        const float rb = a.adjoint ? B[q] : fmaf(dh[q], A[q], B[q]);
+        const float d0 = fmaf(k1, dp[q], k2[q] * ra) + inj[q];
+        const float d1 = fmaf(k1, dr[q], k2[q] * rb) + inj[q];
+        const bool in = (jz + q) < L.Pz;
+        dpn[q] = in ? d0 : 0.f;
+        drn[q] = in ? d1 : 0.f;
+        pn[q] = in ? pc[q] + d0 : 0.f;
+        rn[q] = in ? rc[q] + d1 : 0.f;
+        pr[q] = 0.5f * (pn[q] + rn[q]);
+    }
+    st4(a.d0 + off, make_float4(dpn[0], dpn[1], dpn[2], dpn[3]));
+    st4(a.d1 + off, make_float4(drn[0], drn[1], drn[2], drn[3]));
+    st4(a.n0 + off, make_float4(pn[0], pn[1], pn[2], pn[3]));
+    st4(a.n1 + off, make_float4(rn[0], rn[1], rn[2], rn[3]));
+
+    if (a.PZ != nullptr) {
+        const int ix = jx - L.nb, iz = jz - L.nb;
+        if (ix >= 0 && ix < L.nx && iz >= 0 && iz < L.nz)
+            probe_quad(a.PZ + (long long)ix * L.upz + iz, L.Nu, a.Zrow, a.r, make_float4(pr[0], pr[1], pr[2], pr[3]));
+    }
+}
+
+}  // namespace rtm

@@ -1,0 +1,94 @@
+"""-m gpu: error behaviour of the C ABI (include/rtm.h) on a device."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import rtm_inputs as ri
+
+pytestmark = pytest.mark.gpu
+
+
+def _mk(p, **kw):
+    from paper_2201_06914_b200 import Rtm
+    m = Rtm.from_problem(p, **kw)
+    return m
+
+
+def test_state_and_argument_errors():
+    import torch
+    from paper_2201_06914_b200 import RTMError
+    p = ri.random_acoustic(2, n=(30, 28), nb=4, nt=10, r=2)
+    m = _mk(p)
+    with pytest.raises(RTMError) as e:          # no model / probes yet
+        m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    assert e.value.code == -4
+    m.set_model_from_earth(p.vp)
+    m.set_probes(p.Z)
+    with pytest.raises(RTMError) as e:          # adjoint image before forward
+        m.adjoint_image(p.rec_xyz, np.zeros((p.nt, len(p.rec_xyz)), np.float32), p.src_xyz)
+    assert e.value.code == -4
+    bad = p.src_xyz.copy()
+    bad[0, 0] = -5.0
+    with pytest.raises(RTMError) as e:          # position outside the physical grid
+        m.forward_probe(bad, p.wav, p.rec_xyz)
+    assert e.value.code == -1
+    bad[0, 0] = (p.n[0] - 1) * p.h + 0.5
+    with pytest.raises(RTMError) as e:
+        m.forward_probe(bad, p.wav, p.rec_xyz)
+    assert e.value.code == -1
+    d = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    with pytest.raises(RTMError) as e:          # gather before adjoint
+        m.offset_gather(np.array([0], np.int32))
+    assert e.value.code == -4
+    m.adjoint_image(p.rec_xyz, d, p.src_xyz)
+    with pytest.raises(RTMError) as e:          # |h| >= nx
+        m.offset_gather(np.array([p.n[0]], np.int32))
+    assert e.value.code == -1
+    many = np.tile(p.rec_xyz, (4, 1))           # more points than max_pts
+    with pytest.raises(RTMError) as e:
+        m.forward_probe(p.src_xyz, p.wav, many)
+    assert e.value.code == -1
+    torch.cuda.synchronize()
+    m.close()
+
+
+def test_create_errors():
+    import torch
+    from paper_2201_06914_b200 import binding as B
+    lib = B.load_library()
+    cfg = B.make_config(2, (20, 20), 10.0, 4, 0, 5, 1e-3, 2, 4)
+    need = B.workspace_bytes(cfg)
+    assert need > 0
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    h = C.c_void_p()
+    assert lib.rtm_create(C.byref(cfg), ws.data_ptr(), need - 1, C.byref(h)) == -2          # ENOMEM
+    assert lib.rtm_create(C.byref(cfg), ws.data_ptr() + 4, need, C.byref(h)) == -1          # misaligned
+    assert lib.rtm_create(C.byref(cfg), None, need, C.byref(h)) == -1
+    host = np.zeros(need + 256, np.uint8)
+    hp = (host.ctypes.data + 255) // 256 * 256
+    assert lib.rtm_create(C.byref(cfg), hp, need, C.byref(h)) == -1                          # host pointer
+    for bad in (dict(nb=3), dict(ndim=4), dict(physics=1, ndim=3), dict(r=0), dict(nt=0)):
+        c2 = B.make_config(bad.get("ndim", 2), (20, 20, 20), 10.0, bad.get("nb", 4), bad.get("physics", 0),
+                           bad.get("nt", 5), 1e-3, bad.get("r", 2), 4)
+        assert B.workspace_bytes(c2) == 0
+    assert lib.rtm_create(C.byref(cfg), ws.data_ptr(), need, C.byref(h)) == 0
+    lib.rtm_destroy(h)
+
+
+def test_no_receivers_and_no_image():
+    """Degenerate calls: nrec = 0 forward (probing only), adjoint without image output."""
+    import torch
+    p = ri.random_acoustic(2, n=(30, 28), nb=4, nt=12, r=3)
+    m = _mk(p)
+    m.set_model_from_earth(p.vp)
+    m.set_probes(p.Z)
+    out = m.forward_probe(p.src_xyz, p.wav, np.zeros((0, 2), np.float32), data_out=None)
+    assert out is None
+    uz = m.export_probes(0).cpu().numpy()
+    assert np.abs(uz).max() > 0
+    din = np.ones((p.nt, len(p.rec_xyz)), np.float32)
+    img, q = m.adjoint_image(p.rec_xyz, din, p.src_xyz, image=None)
+    assert img is None
+    torch.cuda.synchronize()
+    m.close()

@@ -1,0 +1,122 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs and probe draws.  Tolerances are north_star's: relative L2 1e-5 for wavefields and receiver
+data, 1e-4 for images and offset gathers (fp32)."""
+import numpy as np
+import pytest
+
+import rtm_inputs as ri
+from gpu_util import check_all, rel, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def test_c0_full():
+    p = ri.make_c0()
+    g, o, e = check_all(p, snap_steps=[50, 150, 250, 350, 499], offsets=np.arange(-5, 6, dtype=np.int32))
+    # coefficient arrays the library computed == the oracle's, bit for bit (reading C18)
+    assert np.array_equal(g["coef"][0], o["co"].K2) and np.array_equal(g["coef"][5], o["co"].damp)
+
+
+def test_c0_exact_image_with_identity_probes():
+    """north_star check 1 on the GPU: r = nt, Z = sqrt(nt) I reproduces sum_t u v of the stored history."""
+    import oracle as orc
+    p = ri.make_c0(nt=120, r=120, n=(41, 37), nb=12)
+    p.Z = ri.identity_probes(p.nt)
+    g = run_gpu(p)
+    co = orc.coeffs(p)
+    f = orc.forward(p, co, want_hist=True)
+    a = orc.adjoint(p, co, g["din"], want_hist=True)
+    Iex = orc.exact_image(f["hist"], a["hist"]) * (float(p.Z[0, 0]) ** 2 / p.nt)
+    assert rel(g["image"], Iex) <= 1e-4
+
+
+@pytest.mark.parametrize("n,nb,r", [((40, 36), 8, 4), ((37, 43), 4, 5), ((33, 30), 0, 1), ((130, 257), 12, 9)])
+def test_acoustic2d_random_offgrid(n, nb, r):
+    p = ri.random_acoustic(2, n=n, nb=nb, nt=80, r=r, seed=3, nsrc=3, nrec=7)
+    check_all(p, snap_steps=[10, 40, 79], offsets=np.array([-3, 0, 2], np.int32))
+
+
+@pytest.mark.parametrize("n,nb,r", [((14, 12, 10), 4, 4), ((21, 18, 37), 8, 3), ((40, 9, 130), 4, 8)])
+def test_acoustic3d_random_offgrid(n, nb, r):
+    p = ri.random_acoustic(3, n=n, nb=nb, nt=50, r=r, seed=4, nsrc=2, nrec=9)
+    check_all(p, snap_steps=[5, 25, 49], offsets=np.array([-2, 0, 1], np.int32))
+
+
+@pytest.mark.parametrize("n,nb,r", [((40, 36), 8, 4), ((75, 131), 12, 7), ((20, 66), 0, 2)])
+def test_tti_random_offgrid(n, nb, r):
+    p = ri.random_tti(n=n, nb=nb, nt=80, r=r, seed=6, nsrc=2, nrec=6)
+    check_all(p, snap_steps=[10, 40, 79], offsets=np.array([-1, 0, 4], np.int32))
+
+
+def test_c1_cropped():
+    p = ri.make_c3(n=(256, 200), nt=600, r=32, nb=80)
+    import oracle as orc
+    # reading C19: adjoint input = F(true) - F(smooth)
+    co_t = orc.coeffs(p, vp=p.vp_true)
+    d_true = orc.forward(p, co_t)["samples"]
+    d_smooth = orc.forward(p, orc.coeffs(p))["samples"]
+    din = (d_true - d_smooth).astype(np.float32)
+    check_all(p, snap_steps=[100, 300, 599], offsets=p.offsets, din=din)
+
+
+def test_c2_cropped():
+    p = ri.make_c2(n=(240, 176), nt=500, r=64, nb=40)
+    check_all(p, snap_steps=[100, 300, 499], offsets=np.array([-4, 0, 4], np.int32))
+
+
+def test_c4_cropped():
+    p = ri.make_c4(n=(72, 64, 56), nt=200, r=16, nb=16, rec_stride=4)
+    check_all(p, snap_steps=[50, 199])
+
+
+def test_gather_h0_equals_image_bitwise():
+    p = ri.random_acoustic(2, n=(50, 45), nb=8, nt=60, r=6, seed=9)
+    g = run_gpu(p, offsets=np.array([0], np.int32))
+    assert np.array_equal(g["gather"][0], g["image"])
+
+
+@pytest.mark.parametrize("make", [
+    lambda: ri.random_acoustic(2, n=(48, 40), nb=8, nt=100, seed=1),
+    lambda: ri.random_acoustic(3, n=(16, 14, 18), nb=4, nt=50, seed=2),
+    lambda: ri.random_tti(n=(44, 40), nb=8, nt=100, seed=3),
+])
+def test_dot_product_on_gpu(make):
+    """north_star check 3: <F q, d> = <q, F^T d> to 1e-5 in fp32."""
+    p = make()
+    rng = np.random.default_rng(17)
+    d = rng.standard_normal((p.nt, len(p.rec_xyz))).astype(np.float32)
+    g = run_gpu(p, din=d)
+    lhs = float((g["data"].astype(np.float64) * d).sum())
+    rhs = float((p.wav.astype(np.float64) * g["qadj"]).sum())
+    nrm = np.linalg.norm(g["data"]) * np.linalg.norm(d)
+    assert abs(lhs - rhs) <= 1e-5 * nrm, (lhs, rhs)
+
+
+def test_run_to_run_repeatable():
+    p = ri.random_acoustic(2, n=(60, 52), nb=8, nt=50, r=4, seed=12)
+    a = run_gpu(p)
+    b = run_gpu(p)
+    for k in ("data", "Uz", "Vz", "image"):
+        assert np.array_equal(a[k], b[k])
+
+
+def test_shot_host_matches_device_calls():
+    import torch
+    from paper_2201_06914_b200 import Rtm
+    p = ri.random_acoustic(2, n=(50, 44), nb=8, nt=60, r=8, seed=13)
+    offs = np.array([-2, 0, 3], np.int32)
+    g = run_gpu(p, offsets=offs)
+    m = Rtm.from_problem(p)
+    m.set_model_from_earth(p.vp)
+    m.set_probes(p.Z)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
+    h_wav, h_din = pin(p.wav), pin(g["din"])
+    h_dout = torch.empty((p.nt, len(p.rec_xyz)), dtype=torch.float32).pin_memory()
+    h_img = torch.empty(p.N, dtype=torch.float32).pin_memory()
+    h_gat = torch.empty((len(offs), p.N), dtype=torch.float32).pin_memory()
+    m.shot_host(p.src_xyz, h_wav, p.rec_xyz, h_din, h_dout, h_img, offs, h_gat)
+    torch.cuda.synchronize()
+    assert np.array_equal(h_dout.numpy(), g["data"])
+    assert np.array_equal(h_img.numpy(), g["image"])
+    assert np.array_equal(h_gat.numpy(), g["gather"])
+    m.close()
