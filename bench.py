@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for BASELINE.json's metric: grid-point updates/s, forward + adjoint with
+fused probing (plus the image and the 41-offset gather: every row of SURVEY.md 8(a)), on configs[1]
+(2D acoustic long-offset subsalt, 1751x751 + 80-pt layer, nt = 6000, r = 32) with configs[3]'s gather.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c1|c2|c4|c0]
+
+A "step" is one shot: rtm_forward_probe + rtm_adjoint_image + rtm_offset_gather.
+value  = N * Np * nt * 2 * K / (max over ranks of the device time of K steps), inputs resident in HBM.
+e2e    = same through rtm_shot_host with pinned HOST buffers (H2D of wavelet + data, D2H of data, image, gather).
+N > 1  = "replicas only" (multi-GPU): every rank runs its own shot, no data-path collective.
+--impl reference times the CPU oracle (as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "grid-point updates/s fwd+adj with fused probing"
+UNIT = "updates/s"
+
+
+def make_problem(name, nt=0):
+    p = _make_problem(name)
+    if nt and nt < p.nt:                          # experiments only
+        p.nt = nt
+        p.wav = np.ascontiguousarray(p.wav[:nt])
+        p.Z = np.ascontiguousarray(p.Z[:nt])
+    return p
+
+
+def _make_problem(name):
+    import rtm_inputs as ri
+    if name == "c1":
+        return ri.make_c3()                     # c1 model/acquisition + c3's 41 offsets
+    if name == "c2":
+        p = ri.make_c2()
+        p.offsets = np.arange(-20, 21, dtype=np.int32)
+        return p
+    if name == "c4":
+        return ri.make_c4()
+    if name == "c0":
+        p = ri.make_c0()
+        p.offsets = np.arange(-20, 21, dtype=np.int32)
+        return p
+    raise SystemExit("unknown workload " + name)
+
+
+def workload_desc(p):
+    return {"workload": {"c3": "configs[1]+configs[3]: 2D acoustic long-offset subsalt + 41-offset gather",
+                         "c2": "configs[2]: 2D TTI", "c4": "configs[4]: 3D acoustic",
+                         "c0": "configs[0]: 2D acoustic small"}.get(p.name, p.name),
+            "grid": list(p.n), "nb": p.nb, "padded_points": p.Np, "nt": p.nt, "r": p.r,
+            "nrec": int(len(p.rec_xyz)), "nh": 0 if p.offsets is None else int(len(p.offsets)),
+            "update_form": "increment (u, du)", "probe": "per-step fused"}
+
+
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def oracle_sample(p, budget_s=15.0, max_steps=None):
+    """Time the oracle, as it stands, on `steps` forward + `steps` adjoint steps of the full grid with
+    fused probing.  Returns (updates/s, steps, seconds, threads)."""
+    import oracle as orc
+    co = orc.coeffs(p)
+    rng = np.random.default_rng(0)
+
+    def run(steps):
+        Z = p.Z[:steps]
+        wav = p.wav[:steps]
+        t0 = time.perf_counter()
+        f = orc.propagate(p, co, False, p.src_xyz, wav, p.rec_xyz, Z=Z, nt=steps)
+        din = np.ascontiguousarray(f["samples"], np.float32)
+        orc.propagate(p, co, True, p.rec_xyz, din, p.src_xyz, Z=Z, nt=steps)
+        return time.perf_counter() - t0
+
+    ta, tb = run(2), run(6)                      # warm-up + calibration (fixed cost vs per-step cost)
+    per = max((tb - ta) / 4.0, 1e-6)
+    fixed = max(ta - 2.0 * per, 0.0)
+    steps = int(max(2, min(p.nt, (budget_s - fixed) / per)))
+    if max_steps:
+        steps = min(steps, max_steps)
+    t = run(steps)
+    return p.Np * steps * 2 / t, steps, t, orc.num_threads()
+
+
+# ---------------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    p = make_problem(args.workload, args.nt)
+    vals = []
+    ncores = None
+    steps_used = None
+    budget = max(3.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for i in range(args.warmup + args.steps):
+        v, st, t, ncores = oracle_sample(p, budget_s=budget)
+        steps_used = st
+        if i >= args.warmup:
+            vals.append((v, t))
+    value = float(np.mean([v for v, _ in vals]))
+    ms = float(np.mean([t for _, t in vals]) * 1e3)
+    sample = "%d forward + %d adjoint steps of the full %s grid with fused probing (r=%d), per bench step" % (
+        steps_used, steps_used, "x".join(map(str, p.n)), p.r)
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_desc(p),
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": ncores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    import __graft_entry__ as g
+    if rank == 0:
+        g.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2201_06914_b200 import Rtm
+
+    p = make_problem(args.workload, args.nt)
+    offs = p.offsets
+    m = Rtm.from_problem(p, device=str(dev))
+    m.set_option("time_steps", 1)
+    # adjoint input (reading C19): F(true model) - F(migration model), computed on the GPU, untimed
+    m.set_probes(p.Z)
+    m.set_model_from_earth(p.vp_true, p.eps, p.delta, p.theta)
+    d_true = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+    d_smooth = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    din = (d_true - d_smooth).contiguous()
+    wav = torch.from_numpy(p.wav).to(dev)
+    data = torch.empty_like(din)
+    image = torch.zeros(p.n, dtype=torch.float32, device=dev)
+    gather = None if offs is None else torch.empty((len(offs),) + tuple(p.n), dtype=torch.float32, device=dev)
+    torch.cuda.synchronize()
+
+    def shot():
+        m.forward_probe(p.src_xyz, wav, p.rec_xyz, data_out=data)
+        m.adjoint_image(p.rec_xyz, din, p.src_xyz, image=image)
+        if offs is not None:
+            m.offset_gather(offs, out=gather)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, k):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(k):
+            fn()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    for _ in range(args.warmup):
+        shot()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = m.launch_count()
+    ms = timed(shot, args.steps)
+    launches = m.launch_count() - l0
+    fwd_ms, adj_ms = m.last_pass_ms(0), m.last_pass_ms(1)
+    clocks = sampler.stop() if rank == 0 else None
+    units = float(p.Np) * p.nt * 2
+    value = world * units * args.steps / (ms * 1e-3)
+
+    # ---- end to end: host buffers through rtm_shot_host ----
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_wav, h_din = pin(p.wav), din.cpu().pin_memory()
+    h_dout = torch.empty((p.nt, len(p.rec_xyz)), dtype=torch.float32).pin_memory()
+    h_img = torch.empty(p.N, dtype=torch.float32).pin_memory()
+    h_gat = None if offs is None else torch.empty((len(offs), p.N), dtype=torch.float32).pin_memory()
+    staging = m.shot_host(p.src_xyz, h_wav, p.rec_xyz, h_din, h_dout, h_img, offs, h_gat)      # warm-up
+    torch.cuda.synchronize()
+    ke = max(1, min(args.steps, 3))
+    ms_e = timed(lambda: m.shot_host(p.src_xyz, h_wav, p.rec_xyz, h_din, h_dout, h_img, offs, h_gat, staging=staging), ke)
+    e2e = world * units * ke / (ms_e * 1e-3)
+    h2d = h_wav.numel() * 4 + h_din.numel() * 4
+    d2h = h_dout.numel() * 4 + h_img.numel() * 4 + (0 if h_gat is None else h_gat.numel() * 4)
+
+    if rank == 0:
+        peak, how = peaks()
+        # dominant kernel = the fused step kernel; algorithmic DRAM bytes per launch (DESIGN.md byte model):
+        # probe planes read + written once (8 r N); wavefields/K2 are L2-resident in 2D (0), streamed in 3D (20 Np)
+        nfield = 2 if p.physics == 1 else 1
+        alg = 8.0 * p.r * p.N + (20.0 * p.Np if p.ndim == 3 else 0.0) * nfield
+        step_ms = (fwd_ms + adj_ms) / (2.0 * p.nt)
+        ach = alg / (step_ms * 1e-3) / 1e9
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(p.name if p.name != "c3" else "c1")
+            except Exception:
+                traffic = None
+        kern = "tti_step_kernel" if p.physics == 1 else "acoustic_step_kernel<%d>" % p.ndim
+        roof = {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": traffic, "peak_source": how, "algorithmic_bytes_per_launch": alg,
+                "avg_launch_ms": step_ms, "share_of_step": (fwd_ms + adj_ms) / (ms / args.steps)}
+        cpu = None
+        if True:
+            v, st, t, cores = oracle_sample(p, budget_s=12.0)
+            cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": "%d forward + %d adjoint steps of the full grid with fused probing (r=%d), %.1f s" % (st, st, p.r, t)}
+        cfg = workload_desc(p)
+        cfg["l2"] = "per-step working set (probe planes %.0f MB) exceeds the 126 MB L2; no flush needed" % (8.0 * p.r * p.N / 1e6)
+        cfg["parallelism"] = "replicas only (one shot per GPU)"
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+               "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg, "clocks": clocks,
+               "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "ms_per_step": ms_e / ke},
+               "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+               "pass_ms": {"forward_steps": fwd_ms, "adjoint_steps": adj_ms}}
+        print(json.dumps(out), flush=True)
+    m.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c1", choices=["c0", "c1", "c2", "c4"])
+    ap.add_argument("--nt", type=int, default=0, help="experiments only: shorten the record (not the headline config)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -125,7 +125,12 @@ int rtm_set_snapshots(rtm_ctx *ctx, int nsnap, const int *h_steps, float *d_out)
 int rtm_export_coeff(rtm_ctx *ctx, int which, float *d_out, void *cuda_stream);
 /* Number of kernels this context has launched so far (bench.py's gpu_launches).                  */
 long long rtm_launch_count(const rtm_ctx *ctx);
-/* Tuning knob: name/value pairs such as "graph" (CUDA-graph the time loop).      */
+/* Device time [ms] of the step-kernel loop (nt launches, excluding the zero-fill and the final
+ * sampling launch) of the last forward (which = 0) / adjoint (which = 1) pass, taken with CUDA events
+ * on that pass's stream when option "time_steps" is 1.  Blocks the host until the pass has finished.
+ * Negative if no timed pass has run.                                                               */
+float rtm_last_pass_ms(rtm_ctx *ctx, int which);
+/* Tuning knob: name/value pairs: "time_steps" (0|1), "graph" (0|1).      */
 int rtm_set_option(rtm_ctx *ctx, const char *name, int value);
 
 const char *rtm_strerror(int code);

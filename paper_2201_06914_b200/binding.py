@@ -15,7 +15,7 @@ _lib = None
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
            "rtm_set_probes", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
-           "rtm_export_coeff", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
+           "rtm_export_coeff", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
 
 
 class RTMError(RuntimeError):
@@ -64,6 +64,8 @@ def load_library():
     lib.rtm_export_coeff.argtypes = [vp, ip, vp, vp]
     lib.rtm_launch_count.restype = C.c_longlong
     lib.rtm_launch_count.argtypes = [vp]
+    lib.rtm_last_pass_ms.restype = C.c_float
+    lib.rtm_last_pass_ms.argtypes = [vp, ip]
     lib.rtm_set_option.argtypes = [vp, C.c_char_p, ip]
     lib.rtm_strerror.restype = C.c_char_p
     lib.rtm_strerror.argtypes = [ip]
@@ -281,6 +283,9 @@ class Rtm:
 
     def launch_count(self) -> int:
         return int(self.lib.rtm_launch_count(self.ctx))
+
+    def last_pass_ms(self, which: int) -> float:
+        return float(self.lib.rtm_last_pass_ms(self.ctx, int(which)))
 
     def set_option(self, name: str, value: int):
         _check(self.lib.rtm_set_option(self.ctx, name.encode(), int(value)))

@@ -66,7 +66,9 @@ struct rtm_ctx {
     std::vector<int> snap_steps;
     float *snap_out;
     long long launches;
-    int opt_graph;
+    int opt_graph, opt_time;
+    cudaEvent_t ev[2][2];
+    bool ev_valid[2];
 };
 
 static bool valid_cfg(const rtm_config *c) {
@@ -195,6 +197,10 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     c->snap_out = nullptr;
     c->launches = 0;
     c->opt_graph = 0;
+    c->opt_time = 0;
+    c->ev_valid[0] = c->ev_valid[1] = false;
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) CU(cudaEventCreate(&c->ev[i][j]));
     c->offs_pending = false;
     const int nc = 1 << cfg->ndim;
     for (int t = 0; t < 2; t++) {
@@ -220,6 +226,8 @@ extern "C" void rtm_destroy(rtm_ctx *c) {
     }
     if (c->offs_done) { cudaEventSynchronize(c->offs_done); cudaEventDestroy(c->offs_done); }
     cudaFreeHost(c->h_offs);
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++) if (c->ev[i][j]) cudaEventDestroy(c->ev[i][j]);
     delete c;
 }
 
@@ -488,6 +496,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     const bool deferred = want_smp && (long long)g.nsmp <= nblocks * 256;
     const unsigned smp_blocks = (unsigned)((g.nsmp + 255) / 256);
 
+    if (c->opt_time) CU(cudaEventRecord(c->ev[adjoint][0], st));
     int cur = 0;
     const long long Np = (long long)L.Px * L.Py * L.Pz;
     for (int step = 0; step < nt; step++) {
@@ -500,6 +509,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
         a.smp_out = (deferred && step > 0) ? d_smp_out + (size_t)nprev * g.nsmp : nullptr;
         launch_step(c, a, grid, block, smem, st);
         cur ^= 1;
+        if (c->opt_time && step == nt - 1) { CU(cudaEventRecord(c->ev[adjoint][1], st)); c->ev_valid[adjoint] = true; }
         if (want_smp && (!deferred || step == nt - 1)) {
             StepArgs s = a;   // sample the field just computed
             s.u0 = c->fld[0][cur]; s.u1 = c->fld[1][cur];
@@ -662,11 +672,20 @@ extern "C" int rtm_export_coeff(rtm_ctx *c, int which, float *d_out, void *strea
     return RTM_OK;
 }
 
+extern "C" float rtm_last_pass_ms(rtm_ctx *c, int which) {
+    if (!c || (which != 0 && which != 1) || !c->ev_valid[which]) return -1.0f;
+    if (cudaEventSynchronize(c->ev[which][1]) != cudaSuccess) return -1.0f;
+    float ms = -1.0f;
+    if (cudaEventElapsedTime(&ms, c->ev[which][0], c->ev[which][1]) != cudaSuccess) return -1.0f;
+    return ms;
+}
+
 extern "C" long long rtm_launch_count(const rtm_ctx *c) { return c ? c->launches : 0; }
 
 extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!c || !name) return RTM_EINVAL;
     if (!strcmp(name, "graph")) { c->opt_graph = value; return RTM_OK; }
+    if (!strcmp(name, "time_steps")) { c->opt_time = value; return RTM_OK; }
     return RTM_EINVAL;
 }
 
