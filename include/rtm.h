@@ -44,6 +44,10 @@ typedef struct {
     double dt;      /* time step [s] (used by rtm_coeffs_host only)                               */
     int r;          /* number of probing vectors, 1..256 (Eq. 1)                    */
     int max_pts;    /* upper bound on nsrc and nrec of any later call (sizes geometry tables)     */
+    int probe_block;/* T_b: 0|1 = probe fused into every time step (8 r bytes/point/step of Uz traffic);
+                       2..16 = time-blocked probing: each step stores its field into a T_b-slot history
+                       ring and every T_b steps one flush applies T_b rows of Z (traffic / T_b).
+                       Same sums, same order per (k,x); costs T_b N floats of workspace.           */
 } rtm_config;
 
 /* Bytes of device workspace rtm_create needs for this config; 0 if the config is invalid.

@@ -27,7 +27,7 @@ class RTMError(RuntimeError):
 class RtmConfig(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("h", C.c_float), ("nb", C.c_int),
                 ("physics", C.c_int), ("nt", C.c_int), ("dt", C.c_double), ("r", C.c_int),
-                ("max_pts", C.c_int)]
+                ("max_pts", C.c_int), ("probe_block", C.c_int)]
 
 
 def lib_path() -> str:
@@ -83,7 +83,7 @@ def _check(rc):
         raise RTMError(rc, "rtm error %d: %s" % (rc, msg))
 
 
-def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts) -> RtmConfig:
+def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block=0) -> RtmConfig:
     c = RtmConfig()
     c.ndim = int(ndim)
     for i, v in enumerate(n):
@@ -95,6 +95,7 @@ def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts) -> RtmConfig:
     c.dt = float(dt)
     c.r = int(r)
     c.max_pts = int(max_pts)
+    c.probe_block = int(probe_block)
     return c
 
 
@@ -127,11 +128,12 @@ def coeffs_host(cfg: RtmConfig, vp, eps=None, delta=None, theta=None):
 class Rtm:
     """One context = one (model, acquisition size) on one GPU.  Same calls as include/rtm.h."""
 
-    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0"):
+    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0", probe_block=0):
         import torch
         self.torch = torch
         self.lib = load_library()
-        self.cfg = make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts)
+        self.cfg = make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block)
+        self.probe_block = int(probe_block)
         self.device = torch.device(device)
         nbytes = workspace_bytes(self.cfg)
         if nbytes == 0:
@@ -148,10 +150,10 @@ class Rtm:
         self._keep = []
 
     @classmethod
-    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None):
+    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None, probe_block=0):
         mp = max(len(p.src_xyz), len(p.rec_xyz)) if max_pts is None else max_pts
         return cls(p.ndim, p.n, p.h, p.nb, p.physics, p.nt if nt is None else nt, p.dt,
-                   p.r if r is None else r, mp, device=device)
+                   p.r if r is None else r, mp, device=device, probe_block=probe_block)
 
     def close(self):
         if getattr(self, "ctx", None):

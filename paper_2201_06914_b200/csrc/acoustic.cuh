@@ -22,6 +22,8 @@ namespace rtm {
 
 template <int ND>
 __global__ void __launch_bounds__(256) acoustic_step_kernel(const StepArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 32 + threadIdx.x;
     const int lin_block = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
@@ -86,10 +88,13 @@ __global__ void __launch_bounds__(256) acoustic_step_kernel(const StepArgs a) {
     const float4 unew = make_float4(un[0], un[1], un[2], un[3]);
     st4(a.n0 + off, unew);
 
-    if (a.PZ != nullptr) {
+    if (a.PZ != nullptr || a.hist != nullptr) {
         const int ix = jx - L.nb, iy = jy - L.nby, iz = jz - L.nb;
-        if (ix >= 0 && ix < L.nx && iy >= 0 && iy < L.ny && iz >= 0 && iz < L.nz)
-            probe_quad(a.PZ + ((long long)ix * L.ny + iy) * L.upz + iz, L.Nu, a.Zrow, a.r, unew);
+        if (ix >= 0 && ix < L.nx && iy >= 0 && iy < L.ny && iz >= 0 && iz < L.nz) {
+            const long long o = ((long long)ix * L.ny + iy) * L.upz + iz;
+            if (a.hist != nullptr) st4(a.hist + o, unew);
+            else probe_quad(a.PZ + o, L.Nu, a.Zrow, a.r, unew);
+        }
     }
 }
 

@@ -47,6 +47,9 @@ struct StepArgs {
     float *PZ;
     const float *Zrow;
     int r;
+    // time-blocked probing: instead of PZ, store the probed field into this history slot (physical grid,
+    // probe-plane layout); probe_flush_kernel applies T rows of Z at once
+    float *hist;
     // fused injection (row-CSR over (jx,jy) rows, restricted to a bounding box)
     const int *row_start;
     const InjEntry *ent;
@@ -75,6 +78,11 @@ __device__ __forceinline__ void st4(float *p, float4 v) { *reinterpret_cast<floa
 // streaming (evict-first) accesses for the probe planes: read once + written once per step
 __device__ __forceinline__ float4 ldcs4(const float *p) { return __ldcs(reinterpret_cast<const float4 *>(p)); }
 __device__ __forceinline__ void stcs4(float *p, float4 v) { __stcs(reinterpret_cast<float4 *>(p), v); }
+
+// Programmatic dependent launch: let the next step's grid become resident while this one drains, and
+// wait for the previous grid (and its memory) before touching anything it wrote.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 __device__ __forceinline__ float k1_of(float s) { return s == 0.0f ? 1.0f : (1.0f - s) / (1.0f + s); }
 

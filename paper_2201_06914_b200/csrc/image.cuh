@@ -108,3 +108,57 @@ __global__ void pack_probes_kernel(int nt, int r, int zr, const float *__restric
 __global__ void __launch_bounds__(256) sample_kernel(const StepArgs a) { sample_points(a, blockIdx.x, 256, threadIdx.x); }
 
 }  // namespace rtm
+
+namespace rtm {
+
+// Time-blocked probe accumulation (a5/a6 with T steps per flush):
+//   PZ[k][x] += sum_{j < ncur} Z[n_j][k] * hist[j][x],   n_j = n_0 + j*dir  (dir = +1 forward, -1 adjoint)
+// Same sums as T per-step rank-1 updates, applied in step order j = 0..ncur-1 per (k, x), so the result does
+// not depend on T's grouping beyond fp32 rounding of the partial sums.  Thread = one physical z-quad; the T
+// history quads stay in registers while the r probe planes stream through once (8 r N bytes per T steps).
+template <int T>
+__global__ void __launch_bounds__(256) probe_flush_kernel(Layout L, const float *__restrict__ hist, int ncur,
+                                                          const float *__restrict__ Z0, long long zstep, int zr,
+                                                          int r, float *__restrict__ PZ) {
+    __shared__ __align__(16) float sz[T * 256];   // [T][zr], zr <= 256
+    for (int i = threadIdx.x; i < T * zr; i += 256) {
+        const int j = i / zr, k = i % zr;
+        sz[i] = j < ncur ? Z0[j * zstep + k] : 0.0f;
+    }
+    __syncthreads();
+    const int nq = L.upz / 4;
+    const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
+    const long long rows = (long long)L.nx * L.ny;
+    if (t >= rows * nq) return;
+    const long long row = t / nq;
+    const int iz = (int)(t % nq) * 4;
+    if (iz >= L.nz) return;
+    const long long o = row * L.upz + iz;
+    float4 h[T];
+#pragma unroll
+    for (int j = 0; j < T; j++) h[j] = j < ncur ? ld4(hist + j * L.Nu + o) : make_float4(0.f, 0.f, 0.f, 0.f);
+    float *p = PZ + o;
+    for (int k = 0; k < r; k += 4) {   // zr is a multiple of 8 and rows beyond r are zero-padded
+        float4 acc[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+            acc[i] = (k + i < r) ? ldcs4(p + (long long)(k + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < T; j++) {
+            const float4 z = ld4(sz + j * zr + k);
+            const float zz[4] = {z.x, z.y, z.z, z.w};
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                acc[i].x = fmaf(zz[i], h[j].x, acc[i].x);
+                acc[i].y = fmaf(zz[i], h[j].y, acc[i].y);
+                acc[i].z = fmaf(zz[i], h[j].z, acc[i].z);
+                acc[i].w = fmaf(zz[i], h[j].w, acc[i].w);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+            if (k + i < r) stcs4(p + (long long)(k + i) * L.Nu, acc[i]);
+    }
+}
+
+}  // namespace rtm

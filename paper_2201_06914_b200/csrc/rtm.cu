@@ -50,8 +50,8 @@ struct rtm_ctx {
     size_t fields_bytes;
     float *K2, *epsh, *delh, *cs, *sn;
     float *dampx, *dampy, *dampz;
-    float *Uz, *Vz, *Zf, *Za;
-    int zr;
+    float *Uz, *Vz, *Zf, *Za, *hist;
+    int zr, T;
     int *row_start;
     InjEntry *ent;
     int *smp_idx;
@@ -66,7 +66,7 @@ struct rtm_ctx {
     std::vector<int> snap_steps;
     float *snap_out;
     long long launches;
-    int opt_graph, opt_time;
+    int opt_graph, opt_time, opt_pdl;
     cudaEvent_t ev[2][2];
     bool ev_valid[2];
 };
@@ -81,6 +81,7 @@ static bool valid_cfg(const rtm_config *c) {
     if (c->physics != 0 && c->physics != 1) return false;
     if (c->physics == 1 && c->ndim != 2) return false;
     if (c->nt < 1 || c->r < 1 || c->r > 256 || c->max_pts < 1) return false;
+    if (c->probe_block < 0 || c->probe_block > 16) return false;
     return true;
 }
 
@@ -126,6 +127,8 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t o_dx = take((size_t)(L.Px + 8) * 4), o_dy = take((size_t)(L.Py + 8) * 4), o_dz = take((size_t)(L.Pz + 8) * 4);
     size_t pb = (size_t)c->r * (size_t)L.Nu * 4;
     size_t o_U = take(pb), o_V = take(pb);
+    const int T = c->probe_block > 1 ? c->probe_block : 0;
+    size_t o_H = take((size_t)T * (size_t)L.Nu * 4);
     const int zr = (int)rup(c->r, 8);
     size_t zb = (size_t)c->nt * zr * 4;
     size_t o_Zf = take(zb), o_Za = take(zb);
@@ -152,6 +155,8 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->dampz = (float *)(b + o_dz);
         ctx->Uz = (float *)(b + o_U);
         ctx->Vz = (float *)(b + o_V);
+        ctx->hist = T ? (float *)(b + o_H) : nullptr;
+        ctx->T = T;
         ctx->Zf = (float *)(b + o_Zf);
         ctx->Za = (float *)(b + o_Za);
         ctx->zr = zr;
@@ -198,6 +203,7 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     c->launches = 0;
     c->opt_graph = 0;
     c->opt_time = 0;
+    c->opt_pdl = 1;
     c->ev_valid[0] = c->ev_valid[1] = false;
     for (int i = 0; i < 2; i++)
         for (int j = 0; j < 2; j++) CU(cudaEventCreate(&c->ev[i][j]));
@@ -452,9 +458,29 @@ static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
 }
 
 static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
-    if (c->cfg.physics == 1) tti_step_kernel<<<grid, block, smem, st>>>(a);
-    else if (c->cfg.ndim == 2) acoustic_step_kernel<2><<<grid, block, 0, st>>>(a);
-    else acoustic_step_kernel<3><<<grid, block, 0, st>>>(a);
+    // programmatic dependent launch: the grid may become resident while its predecessor drains; the
+    // kernels call griddepcontrol.wait before touching memory
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = c->opt_pdl ? 1 : 0;
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    lc.gridDim = grid; lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
+    lc.attrs = at; lc.numAttrs = 1;
+    if (c->cfg.physics == 1) CU(cudaLaunchKernelEx(&lc, tti_step_kernel, a));
+    else if (c->cfg.ndim == 2) CU(cudaLaunchKernelEx(&lc, acoustic_step_kernel<2>, a));
+    else CU(cudaLaunchKernelEx(&lc, acoustic_step_kernel<3>, a));
+    c->launches++;
+    return RTM_OK;
+}
+
+static int launch_flush(rtm_ctx *c, int ncur, const float *Z0, long long zstep, float *PZ, cudaStream_t st) {
+    const Layout &L = c->L;
+    const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
+    const unsigned nb = (unsigned)((tot + 255) / 256);
+    if (c->T <= 4) probe_flush_kernel<4><<<nb, 256, 0, st>>>(L, c->hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    else if (c->T <= 8) probe_flush_kernel<8><<<nb, 256, 0, st>>>(L, c->hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    else probe_flush_kernel<16><<<nb, 256, 0, st>>>(L, c->hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
     c->launches++;
     return RTM_OK;
 }
@@ -463,7 +489,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
                     float *PZ, const float *Z, cudaStream_t st) {
     const rtm_config &cfg = c->cfg;
     const Layout &L = c->L;
-    const int nt = cfg.nt, d = cfg.ndim;
+    const int nt = cfg.nt, d = cfg.ndim, T = c->T;
     CU(cudaMemsetAsync(c->fields_base, 0, c->fields_bytes, st));
     CU(cudaMemsetAsync(PZ, 0, (size_t)cfg.r * (size_t)L.Nu * 4, st));
 
@@ -507,8 +533,14 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
         a.Zrow = Z + (size_t)n * c->zr;
         a.inj_val = d_inj_val + (size_t)n * g.ninj;
         a.smp_out = (deferred && step > 0) ? d_smp_out + (size_t)nprev * g.nsmp : nullptr;
-        launch_step(c, a, grid, block, smem, st);
+        const int slot = T ? step % T : 0;
+        if (T) { a.PZ = nullptr; a.hist = c->hist + (size_t)slot * L.Nu; }
+        { int rc_ = launch_step(c, a, grid, block, smem, st); if (rc_) return rc_; }
         cur ^= 1;
+        if (T && (slot == T - 1 || step == nt - 1)) {
+            const int nfirst = adjoint ? n + slot : n - slot;   // step index of slot 0
+            launch_flush(c, slot + 1, Z + (size_t)nfirst * c->zr, adjoint ? -(long long)c->zr : (long long)c->zr, PZ, st);
+        }
         if (c->opt_time && step == nt - 1) { CU(cudaEventRecord(c->ev[adjoint][1], st)); c->ev_valid[adjoint] = true; }
         if (want_smp && (!deferred || step == nt - 1)) {
             StepArgs s = a;   // sample the field just computed
@@ -686,6 +718,7 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!c || !name) return RTM_EINVAL;
     if (!strcmp(name, "graph")) { c->opt_graph = value; return RTM_OK; }
     if (!strcmp(name, "time_steps")) { c->opt_time = value; return RTM_OK; }
+    if (!strcmp(name, "pdl")) { c->opt_pdl = value; return RTM_OK; }
     return RTM_EINVAL;
 }
 

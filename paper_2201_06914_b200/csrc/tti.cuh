@@ -31,6 +31,8 @@ __global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
     float *P3 = P2 + TTI_GX * TTI_GZ;          // sin g_par
     float *P4 = P3 + TTI_GX * TTI_GZ;          // cos g_par
 
+    pdl_launch_dependents();
+    pdl_wait();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 16 + threadIdx.x;
     const int lin_block = blockIdx.y * gridDim.x + blockIdx.x;
@@ -154,10 +156,14 @@ __global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
     st4(a.n0 + off, make_float4(pn[0], pn[1], pn[2], pn[3]));
     st4(a.n1 + off, make_float4(rn[0], rn[1], rn[2], rn[3]));
 
-    if (a.PZ != nullptr) {
+    if (a.PZ != nullptr || a.hist != nullptr) {
         const int ix = jx - L.nb, iz = jz - L.nb;
-        if (ix >= 0 && ix < L.nx && iz >= 0 && iz < L.nz)
-            probe_quad(a.PZ + (long long)ix * L.upz + iz, L.Nu, a.Zrow, a.r, make_float4(pr[0], pr[1], pr[2], pr[3]));
+        if (ix >= 0 && ix < L.nx && iz >= 0 && iz < L.nz) {
+            const long long o = (long long)ix * L.upz + iz;
+            const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
+            if (a.hist != nullptr) st4(a.hist + o, v);
+            else probe_quad(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+        }
     }
 }
 

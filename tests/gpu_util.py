@@ -18,10 +18,12 @@ def snap_rel(gs, rs):
     return max(np.linalg.norm(gs[i] - rs[i]) for i in range(len(rs))) / den
 
 
-def run_gpu(p, snap_steps=(), din=None, offsets=None, want_qadj=True):
+def run_gpu(p, snap_steps=(), din=None, offsets=None, want_qadj=True, probe_block=0, options=None):
     import torch
     from paper_2201_06914_b200 import Rtm
-    m = Rtm.from_problem(p)
+    m = Rtm.from_problem(p, probe_block=probe_block)
+    for k, v in (options or {}).items():
+        m.set_option(k, v)
     coef = m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
     m.set_probes(p.Z)
     out = {"coef": coef}
@@ -66,8 +68,9 @@ TOL_FIELD = 1e-5   # north_star: wavefields and receiver data
 TOL_IMAGE = 1e-4   # north_star: images, offset gathers (and the compressed wavefields they are made of)
 
 
-def check_all(p, snap_steps=(), offsets=None, din=None, tol_field=TOL_FIELD, tol_image=TOL_IMAGE):
-    g = run_gpu(p, snap_steps=snap_steps, din=din, offsets=offsets)
+def check_all(p, snap_steps=(), offsets=None, din=None, tol_field=TOL_FIELD, tol_image=TOL_IMAGE, probe_block=0,
+              options=None):
+    g = run_gpu(p, snap_steps=snap_steps, din=din, offsets=offsets, probe_block=probe_block, options=options)
     o = run_oracle(p, g["din"], snap_steps=snap_steps, offsets=offsets)
     errs = {}
     errs["data"] = rel(g["data"], o["data"])

@@ -120,3 +120,31 @@ def test_shot_host_matches_device_calls():
     assert np.array_equal(h_img.numpy(), g["image"])
     assert np.array_equal(h_gat.numpy(), g["gather"])
     m.close()
+
+
+@pytest.mark.parametrize("T", [2, 3, 4, 8, 13, 16])
+def test_time_blocked_probing_acoustic2d(T):
+    """probe_block = T: same sums as the per-step fused probe (nt = 83 is not a multiple of any T: ragged last block)."""
+    p = ri.random_acoustic(2, n=(70, 61), nb=8, nt=83, r=6, seed=31, nsrc=2, nrec=5)
+    check_all(p, snap_steps=[40, 82], offsets=np.array([-2, 0, 1], np.int32), probe_block=T)
+
+
+@pytest.mark.parametrize("T", [4, 8])
+def test_time_blocked_probing_3d_and_tti(T):
+    p = ri.random_acoustic(3, n=(21, 18, 37), nb=8, nt=45, r=5, seed=32)
+    check_all(p, snap_steps=[44], probe_block=T)
+    q = ri.random_tti(n=(75, 67), nb=12, nt=77, r=9, seed=33)
+    check_all(q, snap_steps=[76], probe_block=T)
+
+
+def test_c1_cropped_time_blocked():
+    p = ri.make_c3(n=(256, 200), nt=600, r=32, nb=80)
+    check_all(p, snap_steps=[599], offsets=p.offsets, probe_block=8)
+
+
+def test_pdl_off_gives_identical_bits():
+    p = ri.random_acoustic(2, n=(60, 52), nb=8, nt=50, r=4, seed=12)
+    a = run_gpu(p)
+    b = run_gpu(p, options={"pdl": 0})
+    for k in ("data", "Uz", "Vz", "image"):
+        assert np.array_equal(a[k], b[k])
