@@ -201,6 +201,8 @@ def run_ours(args):
     m = Rtm.from_problem(p, device=str(dev), probe_block=args.probe_block)
     m.set_option("time_steps", 1)
     m.set_option("pdl", args.pdl)
+    if args.rx:
+        m.set_option("rx", args.rx)
     # adjoint input (reading C19): F(true model) - F(migration model), computed on the GPU, untimed
     m.set_probes(p.Z)
     m.set_model_from_earth(p.vp_true, p.eps, p.delta, p.theta)
@@ -316,6 +318,7 @@ def main():
     ap.add_argument("--workload", default="c1", choices=["c0", "c1", "c2", "c4"])
     ap.add_argument("--probe-block", type=int, default=0, help="T_b of time-blocked probing (0/1 = per-step fused)")
     ap.add_argument("--pdl", type=int, default=1)
+    ap.add_argument("--rx", type=int, default=0)
     ap.add_argument("--nt", type=int, default=0, help="experiments only: shorten the record (not the headline config)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -50,6 +50,17 @@ struct StepArgs {
     // time-blocked probing: instead of PZ, store the probed field into this history slot (physical grid,
     // probe-plane layout); probe_flush_kernel applies T rows of Z at once
     float *hist;
+    // ... and the leading fl_blocks blocks of every step launch flush one slice (pairs [fl_q0, fl_q1) of
+    // float2 units of the physical grid) of the PREVIOUS time block's history into PZ, so that the
+    // DRAM-bound probe update overlaps the L2/latency-bound stencil inside one launch
+    const float *fl_hist;   // slot 0 of the time block being flushed
+    const float *fl_Z0;     // Z row of that block's slot 0
+    long long fl_zstep;     // +zr forward, -zr adjoint
+    int fl_n;               // slots in that block
+    int fl_blocks;
+    long long fl_q0, fl_q1;
+    int zr;
+    unsigned gx, gy;        // stencil grid extents (the launch grid is 1-D: fl_blocks + gx*gy*gz)
     // fused injection (row-CSR over (jx,jy) rows, restricted to a bounding box)
     const int *row_start;
     const InjEntry *ent;
@@ -83,6 +94,57 @@ __device__ __forceinline__ void stcs4(float *p, float4 v) { __stcs(reinterpret_c
 // wait for the previous grid (and its memory) before touching anything it wrote.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+__device__ __forceinline__ float2 ldcs2(const float *p) { return __ldcs(reinterpret_cast<const float2 *>(p)); }
+__device__ __forceinline__ void stcs2(float *p, float2 v) { __stcs(reinterpret_cast<float2 *>(p), v); }
+
+// Flush role (time-blocked probing): PZ[k][x] += sum_{j<n} Z[n_j][k] hist[j][x] for this block's share of
+// the slice, one float2 of x per thread; T history values stay in registers while r planes stream through.
+template <int TM>
+__device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid, int nthreads, int block) {
+    const Layout &L = a.L;
+    const int zr = a.zr, n = a.fl_n, r = a.r;
+    for (int i = tid; i < TM * zr; i += nthreads) {
+        const int j = i / zr, k = i - j * zr;
+        sz[i] = j < n ? a.fl_Z0[j * a.fl_zstep + k] : 0.0f;
+    }
+    __syncthreads();
+    const int np = L.upz / 2;
+    for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
+        const long long row = t / np;
+        const int iz = (int)(t - row * np) * 2;
+        if (iz >= L.nz) continue;
+        const long long o = row * L.upz + iz;
+        float2 h[TM];
+#pragma unroll
+        for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs2(a.fl_hist + j * L.Nu + o) : make_float2(0.f, 0.f);
+        float *p = a.PZ + o;
+        // software-pipelined over groups of 4 planes: the loads of group g+1 are issued BEFORE the stores
+        // of group g (the compiler cannot hoist them itself: it cannot prove the planes do not alias)
+        float2 nxt[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++) nxt[i] = (i < r) ? ldcs2(p + (long long)i * L.Nu) : make_float2(0.f, 0.f);
+        for (int k = 0; k < r; k += 4) {   // Z rows are zero-padded to zr (multiple of 8)
+            float2 acc[4];
+#pragma unroll
+            for (int i = 0; i < 4; i++) acc[i] = nxt[i];
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+                nxt[i] = (k + 4 + i < r) ? ldcs2(p + (long long)(k + 4 + i) * L.Nu) : make_float2(0.f, 0.f);
+#pragma unroll
+            for (int j = 0; j < TM; j++) {
+                const float4 z = ld4(sz + j * zr + k);
+                acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
+                acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
+                acc[2].x = fmaf(z.z, h[j].x, acc[2].x); acc[2].y = fmaf(z.z, h[j].y, acc[2].y);
+                acc[3].x = fmaf(z.w, h[j].x, acc[3].x); acc[3].y = fmaf(z.w, h[j].y, acc[3].y);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+                if (k + i < r) stcs2(p + (long long)(k + i) * L.Nu, acc[i]);
+        }
+    }
+}
 
 __device__ __forceinline__ float k1_of(float s) { return s == 0.0f ? 1.0f : (1.0f - s) / (1.0f + s); }
 
@@ -120,33 +182,32 @@ __device__ __forceinline__ void inject_quad(const StepArgs &a, long long row, in
     }
 }
 
-// Fused probe for one z-quad (a5): PZ[k][x] += Z[k] * v for k < r.  p points at plane 0.
+// Fused probe for one z-quad (a5): PZ[k][x] += Z[k] * v for k < r.  p points at plane 0.  Zrow is padded
+// with zeros to a multiple of 8.  Software-pipelined over groups of 4 planes (loads of the next group are
+// issued before the stores of the current one; see flush_role).
 __device__ __forceinline__ void probe_quad(float *p, long long Nu, const float *__restrict__ Zrow, int r, float4 v) {
-    int k = 0;
-    for (; k + 8 <= r; k += 8) {
-        float4 acc[8];
-        float4 za = ldg4(Zrow + k), zb = ldg4(Zrow + k + 4);
-        float z[8] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
+    float4 nxt[4];
 #pragma unroll
-        for (int i = 0; i < 8; i++) acc[i] = ldcs4(p + (long long)(k + i) * Nu);
+    for (int i = 0; i < 4; i++) nxt[i] = (i < r) ? ldcs4(p + (long long)i * Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = 0; k < r; k += 4) {
+        float4 acc[4];
 #pragma unroll
-        for (int i = 0; i < 8; i++) {
+        for (int i = 0; i < 4; i++) acc[i] = nxt[i];
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+            nxt[i] = (k + 4 + i < r) ? ldcs4(p + (long long)(k + 4 + i) * Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 z4 = ldg4(Zrow + k);
+        const float z[4] = {z4.x, z4.y, z4.z, z4.w};
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
             acc[i].x = fmaf(z[i], v.x, acc[i].x);
             acc[i].y = fmaf(z[i], v.y, acc[i].y);
             acc[i].z = fmaf(z[i], v.z, acc[i].z);
             acc[i].w = fmaf(z[i], v.w, acc[i].w);
         }
 #pragma unroll
-        for (int i = 0; i < 8; i++) stcs4(p + (long long)(k + i) * Nu, acc[i]);
-    }
-    for (; k < r; k++) {
-        float z = __ldg(Zrow + k);
-        float4 acc = ldcs4(p + (long long)k * Nu);
-        acc.x = fmaf(z, v.x, acc.x);
-        acc.y = fmaf(z, v.y, acc.y);
-        acc.z = fmaf(z, v.z, acc.z);
-        acc.w = fmaf(z, v.w, acc.w);
-        stcs4(p + (long long)k * Nu, acc);
+        for (int i = 0; i < 4; i++)
+            if (k + i < r) stcs4(p + (long long)(k + i) * Nu, acc[i]);
     }
 }
 

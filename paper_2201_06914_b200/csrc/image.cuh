@@ -138,11 +138,16 @@ __global__ void __launch_bounds__(256) probe_flush_kernel(Layout L, const float 
 #pragma unroll
     for (int j = 0; j < T; j++) h[j] = j < ncur ? ld4(hist + j * L.Nu + o) : make_float4(0.f, 0.f, 0.f, 0.f);
     float *p = PZ + o;
+    float4 nxt[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) nxt[i] = (i < r) ? ldcs4(p + (long long)i * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
     for (int k = 0; k < r; k += 4) {   // zr is a multiple of 8 and rows beyond r are zero-padded
         float4 acc[4];
 #pragma unroll
+        for (int i = 0; i < 4; i++) acc[i] = nxt[i];
+#pragma unroll
         for (int i = 0; i < 4; i++)
-            acc[i] = (k + i < r) ? ldcs4(p + (long long)(k + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+            nxt[i] = (k + 4 + i < r) ? ldcs4(p + (long long)(k + 4 + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
         for (int j = 0; j < T; j++) {
             const float4 z = ld4(sz + j * zr + k);

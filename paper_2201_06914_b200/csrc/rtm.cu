@@ -51,7 +51,7 @@ struct rtm_ctx {
     float *K2, *epsh, *delh, *cs, *sn;
     float *dampx, *dampy, *dampz;
     float *Uz, *Vz, *Zf, *Za, *hist;
-    int zr, T;
+    int zr, T, rx;
     int *row_start;
     InjEntry *ent;
     int *smp_idx;
@@ -70,6 +70,8 @@ struct rtm_ctx {
     cudaEvent_t ev[2][2];
     bool ev_valid[2];
 };
+
+static int pick_rx(rtm_ctx *c);
 
 static bool valid_cfg(const rtm_config *c) {
     if (!c) return false;
@@ -128,7 +130,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t pb = (size_t)c->r * (size_t)L.Nu * 4;
     size_t o_U = take(pb), o_V = take(pb);
     const int T = c->probe_block > 1 ? c->probe_block : 0;
-    size_t o_H = take((size_t)T * (size_t)L.Nu * 4);
+    size_t o_H = take(2 * (size_t)T * (size_t)L.Nu * 4);   // double-buffered history ring
     const int zr = (int)rup(c->r, 8);
     size_t zb = (size_t)c->nt * zr * 4;
     size_t o_Zf = take(zb), o_Za = take(zb);
@@ -204,6 +206,7 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     c->opt_graph = 0;
     c->opt_time = 0;
     c->opt_pdl = 1;
+    c->rx = (cfg->ndim == 2 && cfg->physics == 0 && c->T > 0) ? pick_rx(c) : 0;
     c->ev_valid[0] = c->ev_valid[1] = false;
     for (int i = 0; i < 2; i++)
         for (int j = 0; j < 2; j++) CU(cudaEventCreate(&c->ev[i][j]));
@@ -446,6 +449,13 @@ static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
         *grid = dim3((L.Pz + TTI_TZ - 1) / TTI_TZ, (L.Px + TTI_TX - 1) / TTI_TX, 1);
         *block = dim3(16, 16, 1);
         *smem = TTI_SMEM;
+    } else if (c->cfg.ndim == 2 && c->T > 0) {
+        // streaming kernel: 1-D list of (row chunk, z-quad) tasks, 128 per block; grid.x = blocks,
+        // a.gx is overwritten with the quads per row by run_pass
+        const long long nq = (L.Pz + 3) / 4, nchunk = (L.Px + c->rx - 1) / c->rx;
+        *grid = dim3((unsigned)((nq * nchunk + 127) / 128), 1, 1);
+        *block = dim3(128, 1, 1);
+        *smem = 0;
     } else if (c->cfg.ndim == 2) {
         *grid = dim3((L.Pz + 127) / 128, (L.Px + 7) / 8, 1);
         *block = dim3(32, 8, 1);
@@ -457,7 +467,40 @@ static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
     }
 }
 
-static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+typedef void (*step_fn)(const StepArgs);
+template <int TM>
+static step_fn stream2d_fn(int rx) {
+    return rx <= 2 ? acoustic2d_stream_kernel<TM, 2> : rx <= 4 ? acoustic2d_stream_kernel<TM, 4>
+         : rx <= 8 ? acoustic2d_stream_kernel<TM, 8> : acoustic2d_stream_kernel<TM, 16>;
+}
+static int tm_of(int T);
+
+// Rows per thread of the 2D streaming kernel: the smallest RX in {2,4,8,16} whose grid fits in one wave
+// of resident blocks (most parallelism without a second, nearly empty wave); large problems use 8.
+static int pick_rx(rtm_ctx *c) {
+    const Layout &L = c->L;
+    int dev = 0, nsm = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const int tm = tm_of(c->T);
+    const size_t fsm = (size_t)tm * c->zr * 4;
+    const long long nq = (L.Pz + 3) / 4;
+    const int cand[4] = {2, 4, 8, 16};
+    for (int i = 0; i < 4; i++) {
+        step_fn f = tm <= 4 ? stream2d_fn<4>(cand[i]) : tm <= 8 ? stream2d_fn<8>(cand[i]) : stream2d_fn<16>(cand[i]);
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, 128, fsm) != cudaSuccess) { cudaGetLastError(); continue; }
+        const long long blocks = (nq * ((L.Px + cand[i] - 1) / cand[i]) + 127) / 128;
+        // leave room for the flush-role blocks that share the launch
+        if (blocks + blocks / 8 <= (long long)per_sm * nsm) return cand[i];
+    }
+    return 8;
+}
+
+static int tm_of(int T) { return T <= 0 ? 0 : T <= 4 ? 4 : T <= 8 ? 8 : 16; }
+
+template <typename K>
+static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, dim3 block, size_t smem, cudaStream_t st) {
     // programmatic dependent launch: the grid may become resident while its predecessor drains; the
     // kernels call griddepcontrol.wait before touching memory
     cudaLaunchAttribute at[1];
@@ -465,22 +508,49 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
     at[0].val.programmaticStreamSerializationAllowed = c->opt_pdl ? 1 : 0;
     cudaLaunchConfig_t lc;
     memset(&lc, 0, sizeof lc);
-    lc.gridDim = grid; lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
+    lc.gridDim = dim3(nblocks, 1, 1); lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
     lc.attrs = at; lc.numAttrs = 1;
-    if (c->cfg.physics == 1) CU(cudaLaunchKernelEx(&lc, tti_step_kernel, a));
-    else if (c->cfg.ndim == 2) CU(cudaLaunchKernelEx(&lc, acoustic_step_kernel<2>, a));
-    else CU(cudaLaunchKernelEx(&lc, acoustic_step_kernel<3>, a));
+    CU(cudaLaunchKernelEx(&lc, kernel, a));
     c->launches++;
     return RTM_OK;
 }
 
-static int launch_flush(rtm_ctx *c, int ncur, const float *Z0, long long zstep, float *PZ, cudaStream_t st) {
+// the launch grid is 1-D: a.fl_blocks flush-role blocks first, then the gx*gy*gz stencil blocks
+static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+    const unsigned nb = a.fl_blocks + grid.x * grid.y * grid.z;
+    const int tm = tm_of(c->T);
+    const size_t fsm = (size_t)tm * c->zr * 4;
+    if (c->cfg.physics == 1) {
+        switch (tm) {
+            case 0: return launch_ex(c, tti_step_kernel<0>, a, nb, block, smem, st);
+            case 4: return launch_ex(c, tti_step_kernel<4>, a, nb, block, smem, st);
+            case 8: return launch_ex(c, tti_step_kernel<8>, a, nb, block, smem, st);
+            default: return launch_ex(c, tti_step_kernel<16>, a, nb, block, smem, st);
+        }
+    } else if (c->cfg.ndim == 2) {
+        switch (tm) {
+            case 0: return launch_ex(c, acoustic_step_kernel<2, 0>, a, nb, block, 0, st);
+            case 4: return launch_ex(c, stream2d_fn<4>(c->rx), a, nb, block, fsm, st);
+            case 8: return launch_ex(c, stream2d_fn<8>(c->rx), a, nb, block, fsm, st);
+            default: return launch_ex(c, stream2d_fn<16>(c->rx), a, nb, block, fsm, st);
+        }
+    } else {
+        switch (tm) {
+            case 0: return launch_ex(c, acoustic_step_kernel<3, 0>, a, nb, block, 0, st);
+            case 4: return launch_ex(c, acoustic_step_kernel<3, 4>, a, nb, block, fsm, st);
+            case 8: return launch_ex(c, acoustic_step_kernel<3, 8>, a, nb, block, fsm, st);
+            default: return launch_ex(c, acoustic_step_kernel<3, 16>, a, nb, block, fsm, st);
+        }
+    }
+}
+
+static int launch_flush(rtm_ctx *c, const float *hist, int ncur, const float *Z0, long long zstep, float *PZ, cudaStream_t st) {
     const Layout &L = c->L;
     const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
     const unsigned nb = (unsigned)((tot + 255) / 256);
-    if (c->T <= 4) probe_flush_kernel<4><<<nb, 256, 0, st>>>(L, c->hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
-    else if (c->T <= 8) probe_flush_kernel<8><<<nb, 256, 0, st>>>(L, c->hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
-    else probe_flush_kernel<16><<<nb, 256, 0, st>>>(L, c->hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    if (c->T <= 4) probe_flush_kernel<4><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    else if (c->T <= 8) probe_flush_kernel<8><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    else probe_flush_kernel<16><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
     c->launches++;
     return RTM_OK;
 }
@@ -518,8 +588,14 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     size_t smem;
     step_grid(c, &grid, &block, &smem);
     const long long nblocks = (long long)grid.x * grid.y * grid.z;
+    const long long bthreads = (long long)block.x * block.y * block.z;
+    const long long pairs = (long long)L.nx * L.ny * (L.upz / 2);
+    a.gx = grid.x; a.gy = grid.y;
+    if (c->rx) a.gx = (unsigned)((L.Pz + 3) / 4);   // streaming kernel: quads per row
+    a.zr = c->zr;
+    a.fl_zstep = adjoint ? -(long long)c->zr : (long long)c->zr;
     const bool want_smp = d_smp_out != nullptr && g.nsmp > 0;
-    const bool deferred = want_smp && (long long)g.nsmp <= nblocks * 256;
+    const bool deferred = want_smp && (long long)g.nsmp <= nblocks * bthreads;
     const unsigned smp_blocks = (unsigned)((g.nsmp + 255) / 256);
 
     if (c->opt_time) CU(cudaEventRecord(c->ev[adjoint][0], st));
@@ -533,13 +609,30 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
         a.Zrow = Z + (size_t)n * c->zr;
         a.inj_val = d_inj_val + (size_t)n * g.ninj;
         a.smp_out = (deferred && step > 0) ? d_smp_out + (size_t)nprev * g.nsmp : nullptr;
-        const int slot = T ? step % T : 0;
-        if (T) { a.PZ = nullptr; a.hist = c->hist + (size_t)slot * L.Nu; }
+        a.fl_blocks = 0;
+        if (T) {
+            // time block b = step / T writes history slots [(b&1) T, (b&1) T + T); while it runs, the
+            // previous block is flushed in len_b slices, one per step launch
+            const int b = step / T, slot = step % T;
+            a.hist = c->hist + ((size_t)(b & 1) * T + slot) * L.Nu;
+            if (b >= 1) {
+                const int len_b = std::min(T, nt - b * T);
+                const int pb = b - 1;
+                const int nfirst = adjoint ? nt - 1 - pb * T : pb * T;
+                a.fl_hist = c->hist + (size_t)(pb & 1) * T * L.Nu;
+                a.fl_Z0 = Z + (size_t)nfirst * c->zr;
+                a.fl_n = T;
+                a.fl_q0 = pairs * slot / len_b;
+                a.fl_q1 = pairs * (slot + 1) / len_b;
+                a.fl_blocks = (int)((a.fl_q1 - a.fl_q0 + bthreads - 1) / bthreads);   // one pair per thread
+            }
+        }
         { int rc_ = launch_step(c, a, grid, block, smem, st); if (rc_) return rc_; }
         cur ^= 1;
-        if (T && (slot == T - 1 || step == nt - 1)) {
-            const int nfirst = adjoint ? n + slot : n - slot;   // step index of slot 0
-            launch_flush(c, slot + 1, Z + (size_t)nfirst * c->zr, adjoint ? -(long long)c->zr : (long long)c->zr, PZ, st);
+        if (T && step == nt - 1) {   // the last time block has no following steps to hide behind
+            const int fb = step / T, lenf = nt - fb * T;
+            const int nfirst = adjoint ? nt - 1 - fb * T : fb * T;
+            launch_flush(c, c->hist + (size_t)(fb & 1) * T * L.Nu, lenf, Z + (size_t)nfirst * c->zr, a.fl_zstep, PZ, st);
         }
         if (c->opt_time && step == nt - 1) { CU(cudaEventRecord(c->ev[adjoint][1], st)); c->ev_valid[adjoint] = true; }
         if (want_smp && (!deferred || step == nt - 1)) {
@@ -719,6 +812,11 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!strcmp(name, "graph")) { c->opt_graph = value; return RTM_OK; }
     if (!strcmp(name, "time_steps")) { c->opt_time = value; return RTM_OK; }
     if (!strcmp(name, "pdl")) { c->opt_pdl = value; return RTM_OK; }
+    if (!strcmp(name, "rx")) {   // rows per thread of the 2D streaming kernel (2|4|8|16); 0 = automatic
+        if (!c->rx) return RTM_EINVAL;
+        c->rx = value > 0 ? value : pick_rx(c);
+        return RTM_OK;
+    }
     return RTM_EINVAL;
 }
 

@@ -22,6 +22,7 @@ constexpr int TTI_FX = TTI_TX + 16, TTI_FZ = TTI_TZ + 16;   // field tile (halo 
 constexpr int TTI_GX = TTI_TX + 8, TTI_GZ = TTI_TZ + 8;     // product tile (halo 4)
 constexpr int TTI_SMEM = (2 * TTI_FX * TTI_FZ + 4 * TTI_GX * TTI_GZ) * 4;
 
+template <int TM>
 __global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
     extern __shared__ __align__(16) float smem[];
     float *sA = smem;                          // [FX][FZ]
@@ -35,10 +36,14 @@ __global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
     pdl_wait();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 16 + threadIdx.x;
-    const int lin_block = blockIdx.y * gridDim.x + blockIdx.x;
+    if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
+        flush_role<(TM > 0 ? TM : 1)>(a, smem, tid, 256, blockIdx.x);
+        return;
+    }
+    const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
     sample_points(a, lin_block, 256, tid);
 
-    const int z0 = blockIdx.x * TTI_TZ, x0 = blockIdx.y * TTI_TX;
+    const int z0 = (lin_block % a.gx) * TTI_TZ, x0 = (lin_block / a.gx) * TTI_TX;
 
     // ---- stage 1: (mixed) fields, halo 8 ----
     for (int i = tid; i < TTI_FX * (TTI_FZ / 4); i += 256) {
@@ -156,12 +161,12 @@ __global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
     st4(a.n0 + off, make_float4(pn[0], pn[1], pn[2], pn[3]));
     st4(a.n1 + off, make_float4(rn[0], rn[1], rn[2], rn[3]));
 
-    if (a.PZ != nullptr || a.hist != nullptr) {
+    if (TM > 0 ? (a.hist != nullptr) : (a.PZ != nullptr)) {
         const int ix = jx - L.nb, iz = jz - L.nb;
         if (ix >= 0 && ix < L.nx && iz >= 0 && iz < L.nz) {
             const long long o = (long long)ix * L.upz + iz;
             const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
-            if (a.hist != nullptr) st4(a.hist + o, v);
+            if (TM > 0) stcs4(a.hist + o, v);
             else probe_quad(a.PZ + o, L.Nu, a.Zrow, a.r, v);
         }
     }
