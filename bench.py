@@ -139,9 +139,10 @@ def oracle_sample(p, budget_s=15.0, max_steps=None):
         orc.propagate(p, co, True, p.rec_xyz, din, p.src_xyz, Z=Z, nt=steps)
         return time.perf_counter() - t0
 
-    ta, tb = run(2), run(6)                      # warm-up + calibration (fixed cost vs per-step cost)
-    per = max((tb - ta) / 4.0, 1e-6)
-    fixed = max(ta - 2.0 * per, 0.0)
+    run(2)                                       # warm-up (library load, page faults)
+    ta, tb = run(3), run(15)                     # calibration: fixed cost vs per-step cost
+    per = max((tb - ta) / 12.0, tb / 60.0, 1e-6)  # never trust a per-step estimate below tb/60 (noise)
+    fixed = max(ta - 3.0 * per, 0.0)
     steps = int(max(2, min(p.nt, (budget_s - fixed) / per)))
     if max_steps:
         steps = min(steps, max_steps)
@@ -201,6 +202,8 @@ def run_ours(args):
     m = Rtm.from_problem(p, device=str(dev), probe_block=args.probe_block)
     m.set_option("time_steps", 1)
     m.set_option("pdl", args.pdl)
+    if args.dbg:
+        m.set_option("dbg", args.dbg)
     if args.rx:
         m.set_option("rx", args.rx)
     # adjoint input (reading C19): F(true model) - F(migration model), computed on the GPU, untimed
@@ -319,6 +322,7 @@ def main():
     ap.add_argument("--probe-block", type=int, default=0, help="T_b of time-blocked probing (0/1 = per-step fused)")
     ap.add_argument("--pdl", type=int, default=1)
     ap.add_argument("--rx", type=int, default=0)
+    ap.add_argument("--dbg", type=int, default=0)
     ap.add_argument("--nt", type=int, default=0, help="experiments only: shorten the record (not the headline config)")
     args = ap.parse_args()
     if args.impl == "reference":

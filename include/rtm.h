@@ -134,6 +134,9 @@ long long rtm_launch_count(const rtm_ctx *ctx);
  * on that pass's stream when option "time_steps" is 1.  Blocks the host until the pass has finished.
  * Negative if no timed pass has run.                                                               */
 float rtm_last_pass_ms(rtm_ctx *ctx, int which);
+/* Timing experiments (option "dbg" & 16): the first 8 phase time stamps (ns, %globaltimer) of each of the first
+ * nblocks (<= 1024) blocks of the last step launch -> h_out [nblocks][8] (HOST).  Synchronises the device.  */
+int rtm_debug_stamps(rtm_ctx *ctx, unsigned long long *h_out, int nblocks);
 /* Tuning knob: name/value pairs: "time_steps" (0|1), "graph" (0|1).      */
 int rtm_set_option(rtm_ctx *ctx, const char *name, int value);
 

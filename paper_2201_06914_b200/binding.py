@@ -15,7 +15,7 @@ _lib = None
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
            "rtm_set_probes", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
-           "rtm_export_coeff", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
+           "rtm_export_coeff", "rtm_debug_stamps", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
 
 
 class RTMError(RuntimeError):
@@ -62,6 +62,7 @@ def load_library():
     lib.rtm_export_probes.argtypes = [vp, ip, vp, vp]
     lib.rtm_set_snapshots.argtypes = [vp, ip, vp, vp]
     lib.rtm_export_coeff.argtypes = [vp, ip, vp, vp]
+    lib.rtm_debug_stamps.argtypes = [vp, vp, ip]
     lib.rtm_launch_count.restype = C.c_longlong
     lib.rtm_launch_count.argtypes = [vp]
     lib.rtm_last_pass_ms.restype = C.c_float
@@ -281,6 +282,11 @@ class Rtm:
         t = self.torch
         out = t.empty(self.Np, dtype=t.float32, device=self.device)
         _check(self.lib.rtm_export_coeff(self.ctx, int(which), self._ptr(out), self._stream()))
+        return out
+
+    def debug_stamps(self, nblocks=1024):
+        out = np.zeros((nblocks, 8), np.uint64)
+        _check(self.lib.rtm_debug_stamps(self.ctx, _hp(out), int(nblocks)))
         return out
 
     def launch_count(self) -> int:

@@ -23,16 +23,16 @@ namespace rtm {
 // TM = 0: probe fused into every step (or no probing); TM = 4|8|16: time-blocked probing (history ring +
 // fused flush slices of up to TM slots).
 template <int ND, int TM>
-__global__ void __launch_bounds__(256) acoustic_step_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(256, 4) acoustic_step_kernel(const StepArgs a) {
     extern __shared__ __align__(16) float dyn_smem[];
     pdl_launch_dependents();
-    pdl_wait();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 32 + threadIdx.x;
     if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
         flush_role<(TM > 0 ? TM : 1)>(a, dyn_smem, tid, 256, blockIdx.x);
         return;
     }
+    pdl_wait();
     const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
     sample_points(a, lin_block, 256, tid);
     const unsigned bx = lin_block % a.gx, byz = lin_block / a.gx;
@@ -109,107 +109,3 @@ __global__ void __launch_bounds__(256) acoustic_step_kernel(const StepArgs a) {
 
 }  // namespace rtm
 
-namespace rtm {
-
-// ---- 2D acoustic step, register-blocked streaming along the slow axis (x) -----------------------
-// Thread = one z-quad column segment of RX consecutive rows.  The 9 x-neighbour quads live in a
-// register queue that slides one row per iteration (1 new LDG.128 of u per row instead of 8); the two
-// z-halo quads of the centre row come from L1.  Per row and quad: 5 LDG.128 (u[x+4], z-halo x2, du, K2),
-// 2-3 STG.128, ~150 flops, addresses are compile-time multiples of the row stride.
-// The host picks RX so that the whole grid is resident in ONE wave whenever the problem is small enough
-// (no tail of a second, nearly empty wave) -- see pick_rx() in rtm.cu.
-template <int TM, int RX>
-__global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const StepArgs a) {
-    extern __shared__ __align__(16) float dyn_smem[];
-    pdl_launch_dependents();
-    pdl_wait();
-    const Layout &L = a.L;
-    const int tid = threadIdx.x;
-    if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
-        flush_role<(TM > 0 ? TM : 1)>(a, dyn_smem, tid, 128, blockIdx.x);
-        return;
-    }
-    const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
-    sample_points(a, lin_block, 128, tid);
-    // flattened task index: (row chunk, z-quad) pairs are dealt to consecutive threads, so no lane idles
-    // on a ragged Pz; a.gx = number of z-quads per row
-    const unsigned task = lin_block * 128u + tid;
-    const unsigned chunk = task / a.gx;
-    const int jz = (int)(task - chunk * a.gx) * 4;
-    const int x0 = (int)chunk * RX;
-    if (x0 >= L.Px) return;
-
-    const int sx = (int)L.sx;
-    const int base = (int)L.org + jz;            // fsize < 2^31 (checked at create)
-    const float *uc = a.u0 + base;
-    float4 q[8 + RX];
-#pragma unroll
-    for (int i = 0; i < 8; i++) q[i] = ld4(uc + (x0 - 4 + i) * sx);
-    const float4 dz4 = ld4(a.dampz + jz);
-    const float dzv[4] = {dz4.x, dz4.y, dz4.z, dz4.w};
-    const bool zdamp = (dz4.x != 0.f) | (dz4.y != 0.f) | (dz4.z != 0.f) | (dz4.w != 0.f);
-    const bool full = jz + 3 < L.Pz;
-    const int iz = jz - L.nb;
-    const bool zphys = iz >= 0 && iz < L.nz;
-
-#pragma unroll
-    for (int rr = 0; rr < RX; rr++) {
-        const int jx = x0 + rr;
-        if (jx >= L.Px) break;
-        const int off = base + jx * sx;
-        q[8 + rr] = ld4(uc + (jx + 4) * sx);
-        const float4 c = q[4 + rr];
-        const float4 zm = ld4(a.u0 + off - 4), zp = ld4(a.u0 + off + 4);
-        const float4 k24 = ld4(a.K2 + off);
-        const float4 du4 = ld4(a.d0 + off);
-        const float win[12] = {zm.x, zm.y, zm.z, zm.w, c.x, c.y, c.z, c.w, zp.x, zp.y, zp.z, zp.w};
-        const float cc[4] = {c.x, c.y, c.z, c.w};
-        float lap[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-        for (int j = 4; j >= 1; j--) {
-            const float4 P = q[4 + rr + j], M = q[4 + rr - j];
-            const float xs[4] = {(P.x - c.x) + (M.x - c.x), (P.y - c.y) + (M.y - c.y),
-                                 (P.z - c.z) + (M.z - c.z), (P.w - c.w) + (M.w - c.w)};
-            const float w = w2(j);
-#pragma unroll
-            for (int e = 0; e < 4; e++) {
-                const float s = ((win[4 + e + j] - cc[e]) + (win[4 + e - j] - cc[e])) + xs[e];
-                lap[e] = fmaf(w, s, lap[e]);
-            }
-        }
-        const float k2[4] = {k24.x, k24.y, k24.z, k24.w};
-        const float du[4] = {du4.x, du4.y, du4.z, du4.w};
-        float d[4];
-        const float sxd = a.dampx[jx];
-        if (sxd == 0.f && !zdamp) {
-#pragma unroll
-            for (int e = 0; e < 4; e++) d[e] = fmaf(k2[e], lap[e], du[e]);          // K1 = 1 exactly
-        } else {
-#pragma unroll
-            for (int e = 0; e < 4; e++) d[e] = fmaf(k1_of(sxd + dzv[e]), du[e], k2[e] * lap[e]);
-        }
-        if (jx >= a.bx0 && jx <= a.bx1 && jz + 3 >= a.bz0 && jz <= a.bz1) {
-            float inj[4] = {0.f, 0.f, 0.f, 0.f};
-            inject_quad(a, jx, jz, k2, inj);
-#pragma unroll
-            for (int e = 0; e < 4; e++) d[e] += inj[e];
-        }
-        float4 dn = make_float4(d[0], d[1], d[2], d[3]);
-        float4 un = make_float4(cc[0] + d[0], cc[1] + d[1], cc[2] + d[2], cc[3] + d[3]);
-        if (!full) {   // ragged quad at the end of a row: keep the halo zero
-            if (jz + 1 >= L.Pz) { dn.y = 0.f; un.y = 0.f; }
-            if (jz + 2 >= L.Pz) { dn.z = 0.f; un.z = 0.f; }
-            dn.w = 0.f; un.w = 0.f;
-        }
-        st4(a.d0 + off, dn);
-        st4(a.n0 + off, un);
-        const int ix = jx - L.nb;
-        if (zphys && ix >= 0 && ix < L.nx) {
-            const long long o = (long long)ix * L.upz + iz;
-            if (TM > 0) { if (a.hist != nullptr) stcs4(a.hist + o, un); }
-            else if (a.PZ != nullptr) probe_quad(a.PZ + o, L.Nu, a.Zrow, a.r, un);
-        }
-    }
-}
-
-}  // namespace rtm

@@ -42,7 +42,10 @@ struct StepArgs {
     float *d0, *d1;         // increment(s) du = u_cur - u_prev, updated in place
     const float *K2, *epsh, *delh, *cs, *sn;
     const float *dampx, *dampy, *dampz;
+    const float *k1x, *k1y, *k1z;   // per-axis K1 tables: k1a[j] = (1 - damp_a[j]) / (1 + damp_a[j])
     int adjoint;
+    int dbg;
+    unsigned long long *dbg_ts;   // timing experiments (dbg & 16): per-phase %globaltimer stamps, [block][8]
     // fused probe: PZ[k][x] += Zrow[k] * new[x]
     float *PZ;
     const float *Zrow;
@@ -58,7 +61,7 @@ struct StepArgs {
     long long fl_zstep;     // +zr forward, -zr adjoint
     int fl_n;               // slots in that block
     int fl_blocks;
-    long long fl_q0, fl_q1;
+    long long fl_q0, fl_q1;   // slice of this launch in units of float2 (flush_role) or float4 (flush_role4)
     int zr;
     unsigned gx, gy;        // stencil grid extents (the launch grid is 1-D: fl_blocks + gx*gy*gz)
     // fused injection (row-CSR over (jx,jy) rows, restricted to a bounding box)
@@ -109,6 +112,7 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
         sz[i] = j < n ? a.fl_Z0[j * a.fl_zstep + k] : 0.0f;
     }
     __syncthreads();
+    pdl_wait();   // the Z rows above are static; the history was written by earlier launches
     const int np = L.upz / 2;
     for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
         const long long row = t / np;
@@ -146,8 +150,66 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
     }
 }
 
-__device__ __forceinline__ float k1_of(float s) { return s == 0.0f ? 1.0f : (1.0f - s) / (1.0f + s); }
+// Same role with one float4 of x per thread (fewer, fatter threads: used by the 2D streaming kernel, whose
+// stencil threads need ~120 registers anyway).  The Z rows are staged BEFORE griddepcontrol.wait (static
+// data); the history of the previous time block is only touched after it.  Pipelined over groups of 2 planes.
+template <int TM>
+__device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int tid, int nthreads, int block) {
+    const Layout &L = a.L;
+    const int zr = a.zr, n = a.fl_n, r = a.r;
+    for (int i = tid; i < TM * zr; i += nthreads) {
+        const int j = i / zr, k = i - j * zr;
+        sz[i] = j < n ? a.fl_Z0[j * a.fl_zstep + k] : 0.0f;
+    }
+    __syncthreads();
+    pdl_wait();
+    const int nq = L.upz / 4;
+    for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
+        const long long row = t / nq;
+        const int iz = (int)(t - row * nq) * 4;
+        if (iz >= L.nz) continue;
+        const long long o = row * L.upz + iz;
+        float4 h[TM];
+#pragma unroll
+        for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs4(a.fl_hist + j * L.Nu + o) : make_float4(0.f, 0.f, 0.f, 0.f);
+        float *p = a.PZ + o;
+        float4 nxt[2];
+#pragma unroll
+        for (int i = 0; i < 2; i++) nxt[i] = (i < r) ? ldcs4(p + (long long)i * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int k = 0; k < r; k += 2) {   // Z rows are zero-padded to zr (multiple of 8)
+            float4 acc[2];
+#pragma unroll
+            for (int i = 0; i < 2; i++) acc[i] = nxt[i];
+#pragma unroll
+            for (int i = 0; i < 2; i++)
+                nxt[i] = (k + 2 + i < r) ? ldcs4(p + (long long)(k + 2 + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int j = 0; j < TM; j++) {
+                const float2 z = *reinterpret_cast<const float2 *>(sz + j * zr + k);
+                acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
+                acc[0].z = fmaf(z.x, h[j].z, acc[0].z); acc[0].w = fmaf(z.x, h[j].w, acc[0].w);
+                acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
+                acc[1].z = fmaf(z.y, h[j].z, acc[1].z); acc[1].w = fmaf(z.y, h[j].w, acc[1].w);
+            }
+#pragma unroll
+            for (int i = 0; i < 2; i++)
+                if (k + i < r) stcs4(p + (long long)(k + i) * L.Nu, acc[i]);
+        }
+    }
+}
 
+__device__ __forceinline__ unsigned long long gtimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define DBG_STAMP(a, slot)                                                                  \
+    do {                                                                                    \
+        if (((a).dbg & 16) && threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x < 1024)    \
+            (a).dbg_ts[blockIdx.x * 8 + (slot)] = gtimer();                                 \
+    } while (0)
+
+__device__ __forceinline__ float k1_of(float s) { return s == 0.0f ? 1.0f : (1.0f - s) / (1.0f + s); }
 // Deferred receiver sampling: the first ceil(nsmp/nthreads) blocks (linear order) take one point
 // per thread (a4: d[j] = scale * sum_c w_c u[corner]; TTI samples p + r).
 __device__ __forceinline__ void sample_points(const StepArgs &a, int lin_block, int nthreads, int tid) {

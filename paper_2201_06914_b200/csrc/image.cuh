@@ -104,6 +104,11 @@ __global__ void pack_probes_kernel(int nt, int r, int zr, const float *__restric
     const long long n = t / zr;
     dst[t] = k < r ? src[n * r + k] : 0.0f;
 }
+// per-axis K1 table: k1[j] = (1 - s_j) / (1 + s_j) (1 where s_j = 0), same arithmetic as k1_of in the step kernels
+__global__ void k1_table_kernel(const float *__restrict__ damp, float *__restrict__ k1, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) k1[i] = k1_of(damp[i]);
+}
 // stand-alone sampling of the current field (the last step of a pass has no following step kernel)
 __global__ void __launch_bounds__(256) sample_kernel(const StepArgs a) { sample_points(a, blockIdx.x, 256, threadIdx.x); }
 

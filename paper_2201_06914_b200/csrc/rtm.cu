@@ -9,6 +9,8 @@
 
 #include "../../include/rtm.h"
 #include "acoustic.cuh"
+#include "acoustic2d_stream.cuh"
+#include "acoustic3d_stream.cuh"
 #include "image.cuh"
 #include "tti.cuh"
 
@@ -50,6 +52,7 @@ struct rtm_ctx {
     size_t fields_bytes;
     float *K2, *epsh, *delh, *cs, *sn;
     float *dampx, *dampy, *dampz;
+    float *k1x, *k1y, *k1z;
     float *Uz, *Vz, *Zf, *Za, *hist;
     int zr, T, rx;
     int *row_start;
@@ -57,6 +60,7 @@ struct rtm_ctx {
     int *smp_idx;
     float *smp_w;
     int *offs;
+    unsigned long long *dbg_ts;
     long long nrows;
     bool have_model, have_probes, have_U, have_V;
     HostTables ht[2];       // [0] forward call, [1] adjoint call
@@ -66,12 +70,15 @@ struct rtm_ctx {
     std::vector<int> snap_steps;
     float *snap_out;
     long long launches;
-    int opt_graph, opt_time, opt_pdl;
+    int opt_graph, opt_time, opt_pdl, opt_dbg;
     cudaEvent_t ev[2][2];
     bool ev_valid[2];
 };
 
 static int pick_rx(rtm_ctx *c);
+static size_t stream_smem(const rtm_ctx *c, int rx);
+static long long stream_blocks(const rtm_ctx *c, int rx);
+static int tm_of(int T);
 
 static bool valid_cfg(const rtm_config *c) {
     if (!c) return false;
@@ -126,7 +133,8 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t fields_bytes = off - o_fields;
     size_t o_K2 = take(fb), o_e = 0, o_d = 0, o_c = 0, o_s = 0;
     if (nf == 2) { o_e = take(fb); o_d = take(fb); o_c = take(fb); o_s = take(fb); }
-    size_t o_dx = take((size_t)(L.Px + 8) * 4), o_dy = take((size_t)(L.Py + 8) * 4), o_dz = take((size_t)(L.Pz + 8) * 4);
+    size_t o_dx = take((size_t)(L.Px + 32) * 4), o_dy = take((size_t)(L.Py + 8) * 4), o_dz = take((size_t)(L.Pz + 8) * 4);
+    size_t o_kx = take((size_t)(L.Px + 32) * 4), o_ky = take((size_t)(L.Py + 8) * 4), o_kz = take((size_t)(L.Pz + 8) * 4);
     size_t pb = (size_t)c->r * (size_t)L.Nu * 4;
     size_t o_U = take(pb), o_V = take(pb);
     const int T = c->probe_block > 1 ? c->probe_block : 0;
@@ -140,6 +148,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t o_en = take((size_t)c->max_pts * nc * sizeof(InjEntry));
     size_t o_si = take((size_t)c->max_pts * nc * 4), o_sw = take((size_t)c->max_pts * nc * 4);
     size_t o_of = take(4096 * 4);
+    size_t o_dbg = take(1024 * 8 * 8);
     if (ctx) {
         char *b = ctx->ws;
         ctx->nf = nf;
@@ -155,6 +164,9 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->dampx = (float *)(b + o_dx);
         ctx->dampy = (float *)(b + o_dy);
         ctx->dampz = (float *)(b + o_dz);
+        ctx->k1x = (float *)(b + o_kx);
+        ctx->k1y = (float *)(b + o_ky);
+        ctx->k1z = (float *)(b + o_kz);
         ctx->Uz = (float *)(b + o_U);
         ctx->Vz = (float *)(b + o_V);
         ctx->hist = T ? (float *)(b + o_H) : nullptr;
@@ -167,6 +179,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->smp_idx = (int *)(b + o_si);
         ctx->smp_w = (float *)(b + o_sw);
         ctx->offs = (int *)(b + o_of);
+        ctx->dbg_ts = (unsigned long long *)(b + o_dbg);
         ctx->nrows = nrows;
     }
     return off;
@@ -206,6 +219,7 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     c->opt_graph = 0;
     c->opt_time = 0;
     c->opt_pdl = 1;
+    c->opt_dbg = 0;
     c->rx = (cfg->ndim == 2 && cfg->physics == 0 && c->T > 0) ? pick_rx(c) : 0;
     c->ev_valid[0] = c->ev_valid[1] = false;
     for (int i = 0; i < 2; i++)
@@ -331,6 +345,12 @@ extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh,
         t += L.Py;
     }
     CU(cudaMemcpyAsync(c->dampz, t, (size_t)L.Pz * 4, cudaMemcpyHostToDevice, st));
+    // per-axis K1 tables, computed on the device with the same division the kernels use at layer corners
+    k1_table_kernel<<<(L.Px + 32 + 255) / 256, 256, 0, st>>>(c->dampx, c->k1x, L.Px + 32);
+    k1_table_kernel<<<(L.Py + 8 + 255) / 256, 256, 0, st>>>(c->dampy, c->k1y, L.Py + 8);
+    k1_table_kernel<<<(L.Pz + 8 + 255) / 256, 256, 0, st>>>(c->dampz, c->k1z, L.Pz + 8);
+    c->launches += 3;
+    CU(cudaGetLastError());
     c->have_model = true;
     c->have_U = c->have_V = false;
     return RTM_OK;
@@ -448,18 +468,22 @@ static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
     if (c->cfg.physics == 1) {
         *grid = dim3((L.Pz + TTI_TZ - 1) / TTI_TZ, (L.Px + TTI_TX - 1) / TTI_TX, 1);
         *block = dim3(16, 16, 1);
-        *smem = TTI_SMEM;
+        *smem = std::max<size_t>((size_t)TTI_SMEM, (size_t)tm_of(c->T) * c->zr * 4);
     } else if (c->cfg.ndim == 2 && c->T > 0) {
         // streaming kernel: 1-D list of (row chunk, z-quad) tasks, 128 per block; grid.x = blocks,
         // a.gx is overwritten with the quads per row by run_pass
-        const long long nq = (L.Pz + 3) / 4, nchunk = (L.Px + c->rx - 1) / c->rx;
-        *grid = dim3((unsigned)((nq * nchunk + 127) / 128), 1, 1);
+        *grid = dim3((unsigned)stream_blocks(c, c->rx), 1, 1);
         *block = dim3(128, 1, 1);
-        *smem = 0;
+        *smem = stream_smem(c, c->rx);
     } else if (c->cfg.ndim == 2) {
         *grid = dim3((L.Pz + 127) / 128, (L.Px + 7) / 8, 1);
         *block = dim3(32, 8, 1);
         *smem = 0;
+    } else if (c->T > 0) {
+        // 2.5D streaming kernel: (y, z) tiles of 8 x 128, chunks of S3_XCH planes along x
+        *grid = dim3((L.Pz + S3_TZ - 1) / S3_TZ, (L.Py + S3_TY - 1) / S3_TY, (L.Px + S3_XCH - 1) / S3_XCH);
+        *block = dim3(256, 1, 1);
+        *smem = std::max<size_t>((size_t)S3_SMEM, (size_t)tm_of(c->T) * c->zr * 4);
     } else {
         *grid = dim3((L.Pz + 127) / 128, (L.Py + 7) / 8, L.Px);
         *block = dim3(32, 8, 1);
@@ -468,31 +492,42 @@ static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
 }
 
 typedef void (*step_fn)(const StepArgs);
+static int tm_of(int T);
+// ---- launch shape of the 2D streaming kernel ---------------------------------------------------------------
+static const size_t kSmemBudget = 56 * 1024;   // per block: four blocks per SM
+static long long stream_blocks(const rtm_ctx *c, int rx) {
+    const Layout &L = c->L;
+    const long long nq = (L.Pz + 3) / 4, nchunk = (L.Px + rx - 1) / rx;
+    return (nq * nchunk + 127) / 128;
+}
+// dynamic shared memory: injection amounts [RX][128] float4 (stencil role) or the Z rows [TM][zr] (flush role),
+// whichever is larger
+static size_t stream_smem(const rtm_ctx *c, int rx) {
+    const int rxt = rx <= 2 ? 2 : rx <= 4 ? 4 : rx <= 8 ? 8 : 16;
+    return std::max<size_t>((size_t)rxt * 128 * 16, (size_t)tm_of(c->T) * c->zr * 4);
+}
 template <int TM>
 static step_fn stream2d_fn(int rx) {
     return rx <= 2 ? acoustic2d_stream_kernel<TM, 2> : rx <= 4 ? acoustic2d_stream_kernel<TM, 4>
          : rx <= 8 ? acoustic2d_stream_kernel<TM, 8> : acoustic2d_stream_kernel<TM, 16>;
 }
-static int tm_of(int T);
-
 // Rows per thread of the 2D streaming kernel: the smallest RX in {2,4,8,16} whose grid fits in one wave
 // of resident blocks (most parallelism without a second, nearly empty wave); large problems use 8.
 static int pick_rx(rtm_ctx *c) {
-    const Layout &L = c->L;
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const int tm = tm_of(c->T);
-    const size_t fsm = (size_t)tm * c->zr * 4;
-    const long long nq = (L.Pz + 3) / 4;
+    // flush-role blocks that share every launch: one float4 of the physical grid per thread, 1/T of it per step
+    const long long quads = (long long)c->L.nx * c->L.ny * (c->L.upz / 4);
+    const long long fblocks = (quads / std::max(1, c->T) + 127) / 128 + 1;
     const int cand[4] = {2, 4, 8, 16};
     for (int i = 0; i < 4; i++) {
         step_fn f = tm <= 4 ? stream2d_fn<4>(cand[i]) : tm <= 8 ? stream2d_fn<8>(cand[i]) : stream2d_fn<16>(cand[i]);
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, 128, fsm) != cudaSuccess) { cudaGetLastError(); continue; }
-        const long long blocks = (nq * ((L.Px + cand[i] - 1) / cand[i]) + 127) / 128;
-        // leave room for the flush-role blocks that share the launch
-        if (blocks + blocks / 8 <= (long long)per_sm * nsm) return cand[i];
+        cudaFuncSetAttribute((const void *)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, 128, stream_smem(c, cand[i])) != cudaSuccess) { cudaGetLastError(); continue; }
+        if (stream_blocks(c, cand[i]) + fblocks <= (long long)per_sm * nsm) return cand[i];
     }
     return 8;
 }
@@ -510,6 +545,14 @@ static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, 
     memset(&lc, 0, sizeof lc);
     lc.gridDim = dim3(nblocks, 1, 1); lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
     lc.attrs = at; lc.numAttrs = 1;
+    if (smem > 48 * 1024) {   // opt in once per kernel
+        static thread_local std::vector<const void *> done;
+        const void *fp = (const void *)kernel;
+        if (std::find(done.begin(), done.end(), fp) == done.end()) {
+            CU(cudaFuncSetAttribute(fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget));
+            done.push_back(fp);
+        }
+    }
     CU(cudaLaunchKernelEx(&lc, kernel, a));
     c->launches++;
     return RTM_OK;
@@ -519,7 +562,6 @@ static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, 
 static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     const unsigned nb = a.fl_blocks + grid.x * grid.y * grid.z;
     const int tm = tm_of(c->T);
-    const size_t fsm = (size_t)tm * c->zr * 4;
     if (c->cfg.physics == 1) {
         switch (tm) {
             case 0: return launch_ex(c, tti_step_kernel<0>, a, nb, block, smem, st);
@@ -530,16 +572,16 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
     } else if (c->cfg.ndim == 2) {
         switch (tm) {
             case 0: return launch_ex(c, acoustic_step_kernel<2, 0>, a, nb, block, 0, st);
-            case 4: return launch_ex(c, stream2d_fn<4>(c->rx), a, nb, block, fsm, st);
-            case 8: return launch_ex(c, stream2d_fn<8>(c->rx), a, nb, block, fsm, st);
-            default: return launch_ex(c, stream2d_fn<16>(c->rx), a, nb, block, fsm, st);
+            case 4: return launch_ex(c, stream2d_fn<4>(c->rx), a, nb, block, smem, st);
+            case 8: return launch_ex(c, stream2d_fn<8>(c->rx), a, nb, block, smem, st);
+            default: return launch_ex(c, stream2d_fn<16>(c->rx), a, nb, block, smem, st);
         }
     } else {
         switch (tm) {
             case 0: return launch_ex(c, acoustic_step_kernel<3, 0>, a, nb, block, 0, st);
-            case 4: return launch_ex(c, acoustic_step_kernel<3, 4>, a, nb, block, fsm, st);
-            case 8: return launch_ex(c, acoustic_step_kernel<3, 8>, a, nb, block, fsm, st);
-            default: return launch_ex(c, acoustic_step_kernel<3, 16>, a, nb, block, fsm, st);
+            case 4: return launch_ex(c, acoustic3d_stream_kernel<4>, a, nb, block, smem, st);
+            case 8: return launch_ex(c, acoustic3d_stream_kernel<8>, a, nb, block, smem, st);
+            default: return launch_ex(c, acoustic3d_stream_kernel<16>, a, nb, block, smem, st);
         }
     }
 }
@@ -568,6 +610,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     a.L = L;
     a.K2 = c->K2; a.epsh = c->epsh; a.delh = c->delh; a.cs = c->cs; a.sn = c->sn;
     a.dampx = c->dampx; a.dampy = c->dampy; a.dampz = c->dampz;
+    a.k1x = c->k1x; a.k1y = c->k1y; a.k1z = c->k1z;
     a.adjoint = adjoint;
     a.PZ = PZ;
     a.r = cfg.r;
@@ -589,7 +632,8 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     step_grid(c, &grid, &block, &smem);
     const long long nblocks = (long long)grid.x * grid.y * grid.z;
     const long long bthreads = (long long)block.x * block.y * block.z;
-    const long long pairs = (long long)L.nx * L.ny * (L.upz / 2);
+    const int fl_vec = c->rx ? 4 : 2;   // floats per flush-role thread (flush_role4 in the 2D streaming kernel)
+    const long long units = (long long)L.nx * L.ny * (L.upz / fl_vec);
     a.gx = grid.x; a.gy = grid.y;
     if (c->rx) a.gx = (unsigned)((L.Pz + 3) / 4);   // streaming kernel: quads per row
     a.zr = c->zr;
@@ -610,6 +654,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
         a.inj_val = d_inj_val + (size_t)n * g.ninj;
         a.smp_out = (deferred && step > 0) ? d_smp_out + (size_t)nprev * g.nsmp : nullptr;
         a.fl_blocks = 0;
+        a.fl_q0 = a.fl_q1 = 0;
         if (T) {
             // time block b = step / T writes history slots [(b&1) T, (b&1) T + T); while it runs, the
             // previous block is flushed in len_b slices, one per step launch
@@ -622,11 +667,14 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
                 a.fl_hist = c->hist + (size_t)(pb & 1) * T * L.Nu;
                 a.fl_Z0 = Z + (size_t)nfirst * c->zr;
                 a.fl_n = T;
-                a.fl_q0 = pairs * slot / len_b;
-                a.fl_q1 = pairs * (slot + 1) / len_b;
-                a.fl_blocks = (int)((a.fl_q1 - a.fl_q0 + bthreads - 1) / bthreads);   // one pair per thread
+                a.fl_q0 = units * slot / len_b;
+                a.fl_q1 = units * (slot + 1) / len_b;
+                a.fl_blocks = (int)((a.fl_q1 - a.fl_q0 + bthreads - 1) / bthreads);   // one unit per thread
             }
         }
+        if ((c->opt_dbg & 3) == 1) a.fl_blocks = 0;
+        a.dbg = c->opt_dbg;
+        a.dbg_ts = c->dbg_ts;
         { int rc_ = launch_step(c, a, grid, block, smem, st); if (rc_) return rc_; }
         cur ^= 1;
         if (T && step == nt - 1) {   // the last time block has no following steps to hide behind
@@ -805,6 +853,14 @@ extern "C" float rtm_last_pass_ms(rtm_ctx *c, int which) {
     return ms;
 }
 
+// timing experiments: copy the per-block phase stamps of the last launch (dbg & 16) to the host; synchronises
+extern "C" int rtm_debug_stamps(rtm_ctx *c, unsigned long long *h_out, int nblocks) {
+    if (!c || !h_out || nblocks < 1 || nblocks > 1024) return RTM_EINVAL;
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(h_out, c->dbg_ts, (size_t)nblocks * 8 * 8, cudaMemcpyDeviceToHost));
+    return RTM_OK;
+}
+
 extern "C" long long rtm_launch_count(const rtm_ctx *c) { return c ? c->launches : 0; }
 
 extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
@@ -812,6 +868,7 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!strcmp(name, "graph")) { c->opt_graph = value; return RTM_OK; }
     if (!strcmp(name, "time_steps")) { c->opt_time = value; return RTM_OK; }
     if (!strcmp(name, "pdl")) { c->opt_pdl = value; return RTM_OK; }
+    if (!strcmp(name, "dbg")) { c->opt_dbg = value; return RTM_OK; }   // timing experiments only: 1 = no flush role, 2 = no stencil
     if (!strcmp(name, "rx")) {   // rows per thread of the 2D streaming kernel (2|4|8|16); 0 = automatic
         if (!c->rx) return RTM_EINVAL;
         c->rx = value > 0 ? value : pick_rx(c);

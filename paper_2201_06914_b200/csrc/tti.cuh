@@ -23,7 +23,7 @@ constexpr int TTI_GX = TTI_TX + 8, TTI_GZ = TTI_TZ + 8;     // product tile (hal
 constexpr int TTI_SMEM = (2 * TTI_FX * TTI_FZ + 4 * TTI_GX * TTI_GZ) * 4;
 
 template <int TM>
-__global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
     extern __shared__ __align__(16) float smem[];
     float *sA = smem;                          // [FX][FZ]
     float *sB = sA + TTI_FX * TTI_FZ;
@@ -33,13 +33,13 @@ __global__ void __launch_bounds__(256) tti_step_kernel(const StepArgs a) {
     float *P4 = P3 + TTI_GX * TTI_GZ;          // cos g_par
 
     pdl_launch_dependents();
-    pdl_wait();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 16 + threadIdx.x;
     if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
         flush_role<(TM > 0 ? TM : 1)>(a, smem, tid, 256, blockIdx.x);
         return;
     }
+    pdl_wait();
     const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
     sample_points(a, lin_block, 256, tid);
 
