@@ -60,7 +60,7 @@ def workload_desc(p):
                          "c0": "configs[0]: 2D acoustic small"}.get(p.name, p.name),
             "grid": list(p.n), "nb": p.nb, "padded_points": p.Np, "nt": p.nt, "r": p.r,
             "nrec": int(len(p.rec_xyz)), "nh": 0 if p.offsets is None else int(len(p.offsets)),
-            "update_form": "increment (u, du)", "probe": "per-step fused"}
+            "update_form": "increment (u, du)"}
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -140,10 +140,13 @@ def oracle_sample(p, budget_s=15.0, max_steps=None):
         return time.perf_counter() - t0
 
     run(2)                                       # warm-up (library load, page faults)
-    ta, tb = run(3), run(15)                     # calibration: fixed cost vs per-step cost
-    per = max((tb - ta) / 12.0, tb / 60.0, 1e-6)  # never trust a per-step estimate below tb/60 (noise)
-    fixed = max(ta - 3.0 * per, 0.0)
-    steps = int(max(2, min(p.nt, (budget_s - fixed) / per)))
+    t2 = run(2)
+    if t2 > 1.0:                                 # large grids: a couple of steps already cost seconds
+        per = t2 / 2.0
+    else:                                        # the per-step cost grows while the wavefield fills the grid
+        cal = 40                                 # (denormals at the front), so calibrate on a longer run and
+        per = 2.0 * run(cal) / cal               # leave a factor 2 for it
+    steps = int(max(2, min(p.nt, budget_s / per)))
     if max_steps:
         steps = min(steps, max_steps)
     t = run(steps)
@@ -178,6 +181,32 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+SM_COUNT, LANES_PER_SM = 148, 128      # B200: fp32 lanes (B200_PROFILING.md / B300_MICROARCH.md unit counts)
+
+
+def byte_model(p, T):
+    """Algorithmic DRAM bytes of ONE step launch.  2D: the wavefields, du and the coefficient
+    arrays are L2-resident (28-66 MB), so only the probe traffic counts; 3D: 20 B per padded point for the fields."""
+    fields = 20.0 * p.Np if p.ndim == 3 else 0.0
+    if T <= 1:
+        return 8.0 * p.r * p.N + fields                       # every probe plane read + written every step
+    return 8.0 * p.r * p.N / T + 8.0 * p.N + fields           # planes every T steps + history slot written and read
+
+
+def op_model(p):
+    """Algorithmic fp32 lane operations (add, mul or fma = 1) of one step launch."""
+    per_pt = {(2, 0): 34.0, (3, 0): 50.0, (2, 1): 110.0}[(p.ndim, p.physics)]
+    return per_pt * p.Np + float(p.r) * p.N                    # stencil + update, and r FMAs per probed point
+
+
+def kernel_name(p, T):
+    if p.physics == 1:
+        return "tti_step_kernel<%d>" % (0 if T <= 1 else 16 if T > 8 else 8 if T > 4 else 4)
+    if T <= 1:
+        return "acoustic_step_kernel<%d, 0>" % p.ndim
+    return "acoustic2d_stream_kernel" if p.ndim == 2 else "acoustic3d_stream_kernel"
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -199,31 +228,8 @@ def run_ours(args):
 
     p = make_problem(args.workload, args.nt)
     offs = p.offsets
-    m = Rtm.from_problem(p, device=str(dev), probe_block=args.probe_block)
-    m.set_option("time_steps", 1)
-    m.set_option("pdl", args.pdl)
-    if args.dbg:
-        m.set_option("dbg", args.dbg)
-    if args.rx:
-        m.set_option("rx", args.rx)
-    # adjoint input (reading C19): F(true model) - F(migration model), computed on the GPU, untimed
-    m.set_probes(p.Z)
-    m.set_model_from_earth(p.vp_true, p.eps, p.delta, p.theta)
-    d_true = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
-    m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
-    d_smooth = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
-    din = (d_true - d_smooth).contiguous()
-    wav = torch.from_numpy(p.wav).to(dev)
-    data = torch.empty_like(din)
-    image = torch.zeros(p.n, dtype=torch.float32, device=dev)
-    gather = None if offs is None else torch.empty((len(offs),) + tuple(p.n), dtype=torch.float32, device=dev)
-    torch.cuda.synchronize()
-
-    def shot():
-        m.forward_probe(p.src_xyz, wav, p.rec_xyz, data_out=data)
-        m.adjoint_image(p.rec_xyz, din, p.src_xyz, image=image)
-        if offs is not None:
-            m.offset_gather(offs, out=gather)
+    T = args.probe_block
+    units = float(p.Np) * p.nt * 2
 
     def barrier():
         if world > 1:
@@ -245,6 +251,41 @@ def run_ours(args):
             ms = float(t.item())
         return ms
 
+    def make_ctx(Tb):
+        m = Rtm.from_problem(p, device=str(dev), probe_block=Tb)
+        m.set_option("time_steps", 1)
+        m.set_option("pdl", args.pdl)
+        if args.dbg:
+            m.set_option("dbg", args.dbg)
+        if args.rx and Tb > 1 and p.ndim == 2 and p.physics == 0:
+            m.set_option("rx", args.rx)
+        m.set_probes(p.Z)
+        return m
+
+    # ---- headline: device-resident inputs --------------------------------------------------------------------
+    m = make_ctx(T)
+    # adjoint input (reading C19): F(true model) - F(migration model), computed on the GPU, untimed
+    m.set_model_from_earth(p.vp_true, p.eps, p.delta, p.theta)
+    d_true = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+    d_smooth = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    din = (d_true - d_smooth).contiguous()
+    del d_true, d_smooth
+    wav = torch.from_numpy(p.wav).to(dev)
+    data = torch.empty_like(din)
+    image = torch.zeros(p.n, dtype=torch.float32, device=dev)
+    gather = None if offs is None else torch.empty((len(offs),) + tuple(p.n), dtype=torch.float32, device=dev)
+    torch.cuda.synchronize()
+
+    def shot_on(mm):
+        def shot():
+            mm.forward_probe(p.src_xyz, wav, p.rec_xyz, data_out=data)
+            mm.adjoint_image(p.rec_xyz, din, p.src_xyz, image=image)
+            if offs is not None:
+                mm.offset_gather(offs, out=gather)
+        return shot
+
+    shot = shot_on(m)
     for _ in range(args.warmup):
         shot()
     sampler = ClockSampler(local)
@@ -255,10 +296,9 @@ def run_ours(args):
     launches = m.launch_count() - l0
     fwd_ms, adj_ms = m.last_pass_ms(0), m.last_pass_ms(1)
     clocks = sampler.stop() if rank == 0 else None
-    units = float(p.Np) * p.nt * 2
     value = world * units * args.steps / (ms * 1e-3)
 
-    # ---- end to end: host buffers through rtm_shot_host ----
+    # ---- end to end: host buffers through rtm_shot_host ------------------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_wav, h_din = pin(p.wav), din.cpu().pin_memory()
     h_dout = torch.empty((p.nt, len(p.rec_xyz)), dtype=torch.float32).pin_memory()
@@ -271,33 +311,61 @@ def run_ours(args):
     e2e = world * units * ke / (ms_e * 1e-3)
     h2d = h_wav.numel() * 4 + h_din.numel() * 4
     d2h = h_dout.numel() * 4 + h_img.numel() * 4 + (0 if h_gat is None else h_gat.numel() * 4)
+    del staging
+    m.close()
+    del m
+    torch.cuda.empty_cache()
+
+    # ---- the other probe variant, same inputs, for the record (north_star's literal per-step fused design when the
+    # headline is time-blocked, and vice versa): 1 warm-up + 2 timed shots ----------------------------------
+    other = None
+    if args.variants:
+        T2 = 0 if T > 1 else 16
+        m2 = make_ctx(T2)
+        m2.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        shot2 = shot_on(m2)
+        shot2()
+        ms2 = timed(shot2, 2)
+        f2, a2 = m2.last_pass_ms(0), m2.last_pass_ms(1)
+        m2.close()
+        del m2
+        other = (T2, ms2 / 2, f2, a2)
 
     if rank == 0:
         peak, how = peaks()
-        # dominant kernel = the fused step kernel; algorithmic DRAM bytes per launch (DESIGN.md byte model):
-        # probe planes read + written once (8 r N); wavefields/K2 are L2-resident in 2D (0), streamed in 3D (20 Np)
-        nfield = 2 if p.physics == 1 else 1
-        alg = 8.0 * p.r * p.N + (20.0 * p.Np if p.ndim == 3 else 0.0) * nfield
-        step_ms = (fwd_ms + adj_ms) / (2.0 * p.nt)
-        ach = alg / (step_ms * 1e-3) / 1e9
-        traffic = None
+        traffic_tab = {}
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get(p.name if p.name != "c3" else "c1")
+                traffic_tab = json.load(open(tpath))
             except Exception:
-                traffic = None
-        kern = "tti_step_kernel" if p.physics == 1 else "acoustic_step_kernel<%d>" % p.ndim
-        roof = {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": traffic, "peak_source": how, "algorithmic_bytes_per_launch": alg,
-                "avg_launch_ms": step_ms, "share_of_step": (fwd_ms + adj_ms) / (ms / args.steps)}
-        cpu = None
-        if True:
-            v, st, t, cores = oracle_sample(p, budget_s=12.0)
-            cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": "%d forward + %d adjoint steps of the full grid with fused probing (r=%d), %.1f s" % (st, st, p.r, t)}
+                traffic_tab = {}
+
+        def roofline(Tb, f_ms, a_ms, shot_ms):
+            alg = byte_model(p, Tb)
+            step_ms = (f_ms + a_ms) / (2.0 * p.nt)
+            ach = alg / (step_ms * 1e-3) / 1e9
+            ops = op_model(p)
+            sm_ghz = (clocks or {}).get("sm_max_mhz") or 1965.0
+            alu_peak = SM_COUNT * LANES_PER_SM * sm_ghz * 1e6 / 1e12           # T lane-ops/s
+            alu_ach = ops / (step_ms * 1e-3) / 1e12
+            name = ("c1" if p.name == "c3" else p.name) + ("_T%d" % Tb if Tb > 1 else "_T0")
+            return {"bound": "hbm", "kernel": kernel_name(p, Tb), "achieved": ach, "peak": peak, "unit": "GB/s",
+                    "frac": ach / peak, "traffic": traffic_tab.get(name), "peak_source": how,
+                    "algorithmic_bytes_per_launch": alg, "avg_launch_ms": step_ms,
+                    "share_of_step": (f_ms + a_ms) / shot_ms,
+                    "alu": {"achieved": alu_ach, "peak": alu_peak, "unit": "T fp32 lane-ops/s", "frac": alu_ach / alu_peak,
+                            "algorithmic_ops_per_launch": ops}}
+
+        roof = roofline(T, fwd_ms, adj_ms, ms / args.steps)
+        v, st, t, cores = oracle_sample(p, budget_s=12.0)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "%d forward + %d adjoint steps of the full grid with fused probing (r=%d), %.1f s" % (st, st, p.r, t)}
         cfg = workload_desc(p)
-        cfg["l2"] = "per-step working set (probe planes %.0f MB) exceeds the 126 MB L2; no flush needed" % (8.0 * p.r * p.N / 1e6)
+        cfg["probe"] = "per-step fused" if T <= 1 else "time-blocked, T=%d (history ring + fused flush role)" % T
+        cfg["l2"] = ("inputs exceed the 126 MB L2 between uses: probe planes %.0f MB (+ history ring %.0f MB); the 2D "
+                     "wavefields are L2-resident by design; no flush needed"
+                     % (8.0 * p.r * p.N / 1e6, 8.0 * max(T, 0) * p.N / 1e6))
         cfg["parallelism"] = "replicas only (one shot per GPU)"
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -306,8 +374,12 @@ def run_ours(args):
                        "ms_per_step": ms_e / ke},
                "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
                "pass_ms": {"forward_steps": fwd_ms, "adjoint_steps": adj_ms}}
+        if other is not None:
+            T2, ms2, f2, a2 = other
+            out["variant"] = {"probe": "per-step fused" if T2 <= 1 else "time-blocked, T=%d" % T2,
+                              "value": world * units / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2,
+                              "roofline": roofline(T2, f2, a2, ms2)}
         print(json.dumps(out), flush=True)
-    m.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -319,7 +391,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c1", choices=["c0", "c1", "c2", "c4"])
-    ap.add_argument("--probe-block", type=int, default=0, help="T_b of time-blocked probing (0/1 = per-step fused)")
+    ap.add_argument("--probe-block", type=int, default=16,
+                    help="T_b of time-blocked probing (default 16; 0/1 = probe fused into every step)")
+    ap.add_argument("--variants", type=int, default=1, help="also time the other probe variant (2 shots)")
     ap.add_argument("--pdl", type=int, default=1)
     ap.add_argument("--rx", type=int, default=0)
     ap.add_argument("--dbg", type=int, default=0)

@@ -1,16 +1,20 @@
-// acoustic3d_stream.cuh -- 3D isotropic acoustic time step (a1) for time-blocked probing: 2.5D blocking.
+// acoustic3d_stream.cuh -- 3D isotropic acoustic time step (a1) for time-blocked probing: 2.5D blocking with an
+// asynchronous shared-memory pipeline.
 //
 // Block = 256 threads = a (y, z) tile of 8 x 128 points, one z-quad (float4) per thread, streaming along the
 // slow axis x over a chunk of S3_XCH planes.
-//   - x neighbours: a 9-deep register queue per thread that slides one plane per iteration (1 new LDG.128 per
-//     plane instead of 8);
-//   - y and z neighbours: the current plane of the tile (+ halo of 4 in y and z) staged in shared memory,
-//     double-buffered, one __syncthreads per plane;
-//   - the operands of plane p+1 (queue head, halo quads, K2, du, damping) are requested before the arithmetic
-//     of plane p.
-// Per plane and quad: 5 LDG.128 + 2 STS.128 + 10 LDS.128 + 3 STG.128 + ~210 flops, against 23 LDG.128 of the
-// plain kernel; DRAM traffic stays at the algorithmic 20 B/point (u, du read; u', du' written; K2) because the
-// x re-reads of neighbouring chunks and the y/z halos hit L2.
+//   - every global read goes through cp.async (LDGSTS, 16 B, zero-fill outside the allocated halo) into rings in
+//     shared memory, S3_D planes ahead of its use: the haloed u tile of plane p+4+D and the K2 / du tiles of
+//     plane p+D are requested while plane p is computed.  The bytes in flight live in shared memory, not in
+//     registers (a register-prefetch version of this kernel kept 64 B per thread in flight and stalled at 59 %
+//     of the DRAM roofline: memory-level parallelism, not instruction issue, was the limit);
+//   - x neighbours: a 9-deep register queue per thread that slides one plane per iteration and is fed from the
+//     ring when a plane arrives;
+//   - y and z neighbours: read from the ring slot of the current plane (halo of 4 in y and z);
+//   - one __syncthreads per plane: it publishes the arrived plane and frees the slot the next request overwrites.
+// Per plane and quad: 5 LDGSTS + 12 LDS.128 + 3 STG.128, arithmetic in packed fp32x2 (FADD2 / FFMA2).  DRAM
+// traffic stays at the algorithmic 20 B/point (u, du read; u', du' written; K2): the x re-reads of neighbouring
+// chunks and the y/z halos hit L2.
 //
 // Fused as in the 2D kernel: damping through per-axis K1 tables, source injection (a3; the block's injection
 // amounts are looked up by all 256 threads in parallel before griddepcontrol.wait), deferred receiver sampling
@@ -24,8 +28,24 @@ constexpr int S3_TY = 8, S3_TZ = 128;
 constexpr int S3_PITCH = S3_TZ + 8;     // floats per smem row: [z halo 4 | 128 | z halo 4]
 constexpr int S3_ROWS = S3_TY + 8;      // y halo 4 on both sides
 constexpr int S3_XCH = 32;              // planes per chunk
+constexpr int S3_D = 3;                 // prefetch distance in planes
+constexpr int S3_NU = 8;                // u ring slots  = 5 + S3_D (planes p .. p+4+D)
+constexpr int S3_NK = 4;                // K2 / du ring slots = S3_D + 1
+constexpr int S3_TILE = S3_ROWS * S3_PITCH;      // floats per haloed u tile
+constexpr int S3_CT = S3_TY * S3_TZ;             // floats per K2 / du tile
 constexpr int S3_INJCAP = 512;          // injection amounts (float4) a block can stage
-constexpr int S3_SMEM = (2 * S3_ROWS * S3_PITCH) * 4 + S3_INJCAP * 16;
+constexpr int S3_SMEM = (S3_NU * S3_TILE + 2 * S3_NK * S3_CT) * 4 + S3_INJCAP * 16;
+static_assert(S3_NU == 5 + S3_D && S3_NK == S3_D + 1, "ring sizes follow the prefetch distance");
+
+// 16-byte asynchronous copy global -> shared; ok == false writes zeros (the source is not read)
+__device__ __forceinline__ void cp_async16(float *dst_smem, const float *src, bool ok) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    const int n = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // sum of the injection entries of padded row `row` that fall into the z-quad starting at jz (a3)
 __device__ __forceinline__ float4 inject_lookup(const StepArgs &a, long long row, int jz) {
@@ -44,7 +64,7 @@ __device__ __forceinline__ float4 inject_lookup(const StepArgs &a, long long row
     return make_float4(acc[0], acc[1], acc[2], acc[3]);
 }
 
-template <int TM>
+template <int TM, bool PK>
 __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_constant__ StepArgs a) {
     extern __shared__ __align__(16) float dyn_smem[];
     const Layout &L = a.L;
@@ -63,8 +83,7 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     const int nplanes = min(S3_XCH, L.Px - x0);
     const bool act = jz < L.Pz && jy < L.Py;
 
-    float *plane = dyn_smem;                                                   // [2][S3_ROWS][S3_PITCH]
-    float4 *injs = reinterpret_cast<float4 *>(dyn_smem + 2 * S3_ROWS * S3_PITCH);   // [S3_INJCAP]
+    float4 *injs = reinterpret_cast<float4 *>(dyn_smem + S3_NU * S3_TILE + 2 * S3_NK * S3_CT);   // [S3_INJCAP], behind the rings
 
     // ---- prologue on static data (before the grid dependency is resolved) ----------------------------------
     // injection: all (plane, row, z-quad) triples of this block's tile that intersect the bounding box of the
@@ -105,7 +124,7 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     float *__restrict__ n0 = a.n0;
     float *d0 = a.d0;
 
-    // what this thread may load: its centre quad (also when it only feeds a neighbour's halo) ...
+    // what this thread may request: its centre quad (also when it only feeds a neighbour's halo) ...
     const bool ld_c = jz + 8 <= L.pz && jy < L.Py + 4;
     // ... one quad of the y halo (rows -4..-1 and 8..11 of the tile) ...
     const int hrow = ty < 4 ? ty : ty + S3_TY;                 // smem row of the halo quad
@@ -119,7 +138,7 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     const long long oc = L.org + (long long)x0 * sx + (long long)jy * L.sy + jz;
     const float *pc = u0 + oc;                                  // centre quad, plane x0
     const float *phh = u0 + L.org + (long long)x0 * sx + (long long)jyh * L.sy + jz;
-    const float *pk = K2 + oc;
+    const float *pkk = K2 + oc;
     float *pd = d0 + oc;
     float *pn = n0 + oc;
     const int iz = jz - L.nb, iy = jy - L.nby;
@@ -127,102 +146,137 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     float *ph = a.hist + (((long long)(x0 - L.nb) * L.ny + iy) * L.upz + iz);   // dereferenced inside the physical grid only
     const long long hstep = (long long)L.ny * L.upz;
 
-    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    float4 q[9];
+    float *Ub = dyn_smem;                                        // [S3_NU][S3_ROWS][S3_PITCH]
+    float *Kb = Ub + S3_NU * S3_TILE;                            // [S3_NK][S3_TY][S3_TZ]
+    float *Db = Kb + S3_NK * S3_CT;
+    const int o_c = (ty + 4) * S3_PITCH + 4 + tx * 4;            // this thread's centre slot inside a u tile
+    const int o_h = hrow * S3_PITCH + 4 + tx * 4;                // its y-halo slot
+    const int o_k = tid * 4;
+    const int last_pl = min(nplanes + 3, L.Px + 3 - x0);         // last plane (relative to x0) any thread needs
+
+    // request the haloed u tile of plane `pl` (relative to x0); planes nobody needs are skipped
+    auto request_u = [&](int pl) {
+        if (pl > last_pl) return;
+        float *t = Ub + (pl & (S3_NU - 1)) * S3_TILE;
+        const long long o = (long long)pl * sx;
+        cp_async16(t + o_c, ld_c ? pc + o : u0, ld_c);
+        cp_async16(t + o_h, ld_h ? phh + o : u0, ld_h);
+        if (zl) cp_async16(t + o_c - 4, ld_z ? pc + o - 4 : u0, ld_z);
+        if (zr_) cp_async16(t + o_c + 4, ld_z ? pc + o + 4 : u0, ld_z);
+    };
+    auto request_kd = [&](int pl) {
+        if (pl >= nplanes || !act) return;
+        const long long o = (long long)pl * sx;
+        cp_async16(Kb + (pl & (S3_NK - 1)) * S3_CT + o_k, pkk + o, true);
+        cp_async16(Db + (pl & (S3_NK - 1)) * S3_CT + o_k, pd + o, true);
+    };
+    // pipeline prologue: S3_D groups; group g of iteration p carries u plane p+4+D and K2/du plane p+D
+    request_u(0); request_u(1); request_u(2); request_u(3); request_u(4);
+    request_kd(0);
+    cp_async_commit();
 #pragma unroll
-    for (int i = 0; i < 9; i++) q[i] = ld_c ? ld4(pc + (i - 4) * sx) : zero4;
-    float4 hy = ld_h ? ld4(phh) : zero4;
-    float4 hz = ld_z ? ld4(pc + (zl ? -4 : 4)) : zero4;
-    float4 k24 = act ? ld4(pk) : zero4, du4 = act ? ld4(pd) : zero4;
-    float sxd = a.dampx[x0], k1x = a.k1x[x0];
+    for (int g = 1; g < S3_D; g++) {
+        request_u(4 + g);
+        request_kd(g);
+        cp_async_commit();
+    }
 
-    float *srow = plane + (ty + 4) * S3_PITCH + 4 + tx * 4;    // this thread's centre slot in buffer 0
-    float *shal = plane + hrow * S3_PITCH + 4 + tx * 4;        // its y-halo slot
-    constexpr int BUF = S3_ROWS * S3_PITCH;
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 q[9];   // planes p-4 .. p+4 of this thread's quad; q[8] is filled from the ring at the top of iteration p
+#pragma unroll
+    for (int i = 0; i < 8; i++) q[i] = ld_c ? ld4(pc + (i - 4) * sx) : zero4;
 
+    typedef V2<PK> V;
+    typedef typename V::T P2;
+    float sxn = a.dampx[x0], k1xn = a.k1x[x0];   // x damping of the next plane, fetched one iteration ahead
 #pragma unroll 1
     for (int p = 0; p < nplanes; p++) {
-        const int b = (p & 1) * BUF;
+        cp_async_wait<S3_D - 1>();   // this thread's requests of groups <= p - D ... p + 0 - D have landed
+        __syncthreads();             // everybody's have; and nobody reads the slots the next request overwrites
+        request_u(p + 4 + S3_D);
+        request_kd(p + S3_D);
+        cp_async_commit();
+
+        const float *U0 = Ub + (p & (S3_NU - 1)) * S3_TILE + o_c;            // current plane, centre slot
+        q[8] = ld4(Ub + ((p + 4) & (S3_NU - 1)) * S3_TILE + o_c);
         const float4 c = q[4];
-        st4(srow + b, c);
-        st4(shal + b, hy);
-        if (zl) st4(srow + b - 4, hz);
-        if (zr_) st4(srow + b + 4, hz);
-        __syncthreads();
+        const float4 k24c = act ? ld4(Kb + (p & (S3_NK - 1)) * S3_CT + o_k) : zero4;
+        const float4 du4c = act ? ld4(Db + (p & (S3_NK - 1)) * S3_CT + o_k) : zero4;
+        const int jx = x0 + p;
+        const float sxc = sxn, k1xc = k1xn;
+        sxn = a.dampx[jx + 1];   // tables are padded: jx + 1 <= Px is readable
+        k1xn = a.k1x[jx + 1];
 
-        const float k2[4] = {k24.x, k24.y, k24.z, k24.w};
-        const float du[4] = {du4.x, du4.y, du4.z, du4.w};
-        const float sxc = sxd, k1xc = k1x;
-        float4 qn = zero4;
-        if (p + 1 < nplanes) {   // operands of plane p+1, requested before the arithmetic of plane p
-            qn = ld_c ? ld4(pc + 5 * sx) : zero4;
-            hy = ld_h ? ld4(phh + sx) : zero4;
-            hz = ld_z ? ld4(pc + sx + (zl ? -4 : 4)) : zero4;
-            if (act) { k24 = ld4(pk + sx); du4 = ld4(pd + sx); }
-            sxd = a.dampx[x0 + p + 1];
-            k1x = a.k1x[x0 + p + 1];
-        }
-
-        const float4 zm = ld4(srow + b - 4), zp = ld4(srow + b + 4);
+        const float4 zm = ld4(U0 - 4), zp = ld4(U0 + 4);
         const float win[12] = {zm.x, zm.y, zm.z, zm.w, c.x, c.y, c.z, c.w, zp.x, zp.y, zp.z, zp.w};
         const float cc[4] = {c.x, c.y, c.z, c.w};
-        float lap[4] = {0.f, 0.f, 0.f, 0.f};
+        // Laplacian in the difference form, two z points per instruction (FADD2 / FFMA2); same operations in
+        // the same order per point as the scalar kernels: s = ((z part + x part) + y part), lap = fma(w, s, lap)
+        const P2 clo = V::mk(c.x, c.y), chi = V::mk(c.z, c.w);
+        P2 llo = V::mk(0.f, 0.f), lhi = llo;
 #pragma unroll
         for (int j = 4; j >= 1; j--) {   // small weights first
             const float4 XP = q[4 + j], XM = q[4 - j];
-            const float4 YP = ld4(srow + b + j * S3_PITCH), YM = ld4(srow + b - j * S3_PITCH);
-            const float xs[4] = {(XP.x - c.x) + (XM.x - c.x), (XP.y - c.y) + (XM.y - c.y),
-                                 (XP.z - c.z) + (XM.z - c.z), (XP.w - c.w) + (XM.w - c.w)};
-            const float ys[4] = {(YP.x - c.x) + (YM.x - c.x), (YP.y - c.y) + (YM.y - c.y),
-                                 (YP.z - c.z) + (YM.z - c.z), (YP.w - c.w) + (YM.w - c.w)};
-            const float w = w2(j);
+            const float4 YP = ld4(U0 + j * S3_PITCH), YM = ld4(U0 - j * S3_PITCH);
+            const P2 xlo = V::dd(V::mk(XP.x, XP.y), V::mk(XM.x, XM.y), clo), xhi = V::dd(V::mk(XP.z, XP.w), V::mk(XM.z, XM.w), chi);
+            const P2 ylo = V::dd(V::mk(YP.x, YP.y), V::mk(YM.x, YM.y), clo), yhi = V::dd(V::mk(YP.z, YP.w), V::mk(YM.z, YM.w), chi);
+            P2 zlo, zhi;
+            if (j % 2 == 0) {   // shifted z windows are register-pair aligned for even shifts only
+                zlo = V::dd(V::mk(win[4 + j], win[5 + j]), V::mk(win[4 - j], win[5 - j]), clo);
+                zhi = V::dd(V::mk(win[6 + j], win[7 + j]), V::mk(win[6 - j], win[7 - j]), chi);
+            } else {
+                float zs[4];
 #pragma unroll
-            for (int e = 0; e < 4; e++) {
-                const float s = (((win[4 + e + j] - cc[e]) + (win[4 + e - j] - cc[e])) + xs[e]) + ys[e];
-                lap[e] = fmaf(w, s, lap[e]);
+                for (int e = 0; e < 4; e++) zs[e] = (win[4 + e + j] - cc[e]) + (win[4 + e - j] - cc[e]);
+                zlo = V::mk(zs[0], zs[1]);
+                zhi = V::mk(zs[2], zs[3]);
             }
+            const float w = w2(j);
+            const P2 ww = V::mk(w, w);
+            llo = V::fma(ww, V::add(V::add(zlo, xlo), ylo), llo);
+            lhi = V::fma(ww, V::add(V::add(zhi, xhi), yhi), lhi);
         }
-        float d[4];
+        const P2 k2lo = V::mk(k24c.x, k24c.y), k2hi = V::mk(k24c.z, k24c.w);
+        const P2 dulo = V::mk(du4c.x, du4c.y), duhi = V::mk(du4c.z, du4c.w);
+        P2 dlo, dhi;
         const float sxy = sxc + syv;
         if (sxy == 0.f && !zdamp) {
-#pragma unroll
-            for (int e = 0; e < 4; e++) d[e] = fmaf(k2[e], lap[e], du[e]);          // K1 = 1 exactly
+            dlo = V::fma(k2lo, llo, dulo);          // K1 = 1 exactly
+            dhi = V::fma(k2hi, lhi, duhi);
         } else {
             // one damping axis: its table; several: (1 - s) / (1 + s) with s = (sx + sy) + sz
             const float k1xy = sxc == 0.f ? k1yv : (syv == 0.f ? k1xc : k1_of(sxy));
+            float k1[4];
 #pragma unroll
-            for (int e = 0; e < 4; e++) {
-                const float k1 = sxy == 0.f ? k1z[e] : (dzv[e] == 0.f ? k1xy : k1_of(sxy + dzv[e]));
-                d[e] = fmaf(k1, du[e], k2[e] * lap[e]);
-            }
+            for (int e = 0; e < 4; e++) k1[e] = sxy == 0.f ? k1z[e] : (dzv[e] == 0.f ? k1xy : k1_of(sxy + dzv[e]));
+            dlo = V::fma(V::mk(k1[0], k1[1]), dulo, V::mul(k2lo, llo));
+            dhi = V::fma(V::mk(k1[2], k1[3]), duhi, V::mul(k2hi, lhi));
         }
-        const int jx = x0 + p;
         if (my_hit && jx >= p0 && jx <= p1) {   // a3: K2 * scale * w * val
             const float4 iv = inj_mode == 1 ? injs[my_inj + (jx - p0) * nzq * nr]
                                             : inject_lookup(a, (long long)jx * L.Py + jy, jz);
-            d[0] = fmaf(k2[0], iv.x, d[0]);
-            d[1] = fmaf(k2[1], iv.y, d[1]);
-            d[2] = fmaf(k2[2], iv.z, d[2]);
-            d[3] = fmaf(k2[3], iv.w, d[3]);
+            dlo = V::fma(k2lo, V::mk(iv.x, iv.y), dlo);
+            dhi = V::fma(k2hi, V::mk(iv.z, iv.w), dhi);
         }
         if (act) {
-            float4 dn = make_float4(d[0], d[1], d[2], d[3]);
-            float4 un = make_float4(cc[0] + d[0], cc[1] + d[1], cc[2] + d[2], cc[3] + d[3]);
+            const P2 ulo = V::add(clo, dlo), uhi = V::add(chi, dhi);
+            float4 dn, un;
+            V::get(dlo, dn.x, dn.y); V::get(dhi, dn.z, dn.w);
+            V::get(ulo, un.x, un.y); V::get(uhi, un.z, un.w);
             if (jz + 3 >= L.Pz) {   // ragged quad at the end of a row: keep the halo zero
                 if (jz + 1 >= L.Pz) { dn.y = 0.f; un.y = 0.f; }
                 if (jz + 2 >= L.Pz) { dn.z = 0.f; un.z = 0.f; }
                 dn.w = 0.f; un.w = 0.f;
             }
-            st4(pd, dn);
-            st4(pn, un);
-            if (phys_yz && (unsigned)(jx - L.nb) < (unsigned)L.nx) stcs4(ph, un);
+            st4(pd + (long long)p * sx, dn);
+            st4(pn + (long long)p * sx, un);
+            if (phys_yz && (unsigned)(jx - L.nb) < (unsigned)L.nx) stcs4(ph + (long long)p * hstep, un);
         }
         // slide the x queue by one plane
 #pragma unroll
         for (int i = 0; i < 8; i++) q[i] = q[i + 1];
-        q[8] = qn;
-        pc += sx; phh += sx; pk += sx; pd += sx; pn += sx; ph += hstep;
     }
+    cp_async_wait<0>();
 }
 
 }  // namespace rtm

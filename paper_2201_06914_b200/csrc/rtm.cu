@@ -545,12 +545,14 @@ static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, 
     memset(&lc, 0, sizeof lc);
     lc.gridDim = dim3(nblocks, 1, 1); lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
     lc.attrs = at; lc.numAttrs = 1;
-    if (smem > 48 * 1024) {   // opt in once per kernel
-        static thread_local std::vector<const void *> done;
+    if (smem > 48 * 1024) {   // opt in to large dynamic shared memory, once per kernel and size
+        static thread_local std::vector<std::pair<const void *, size_t>> done;
         const void *fp = (const void *)kernel;
-        if (std::find(done.begin(), done.end(), fp) == done.end()) {
-            CU(cudaFuncSetAttribute(fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget));
-            done.push_back(fp);
+        bool ok = false;
+        for (auto &d : done) ok = ok || (d.first == fp && d.second >= smem);
+        if (!ok) {
+            CU(cudaFuncSetAttribute(fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            done.push_back({fp, smem});
         }
     }
     CU(cudaLaunchKernelEx(&lc, kernel, a));
@@ -579,9 +581,10 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
     } else {
         switch (tm) {
             case 0: return launch_ex(c, acoustic_step_kernel<3, 0>, a, nb, block, 0, st);
-            case 4: return launch_ex(c, acoustic3d_stream_kernel<4>, a, nb, block, smem, st);
-            case 8: return launch_ex(c, acoustic3d_stream_kernel<8>, a, nb, block, smem, st);
-            default: return launch_ex(c, acoustic3d_stream_kernel<16>, a, nb, block, smem, st);
+            case 4: return launch_ex(c, acoustic3d_stream_kernel<4, true>, a, nb, block, smem, st);
+            case 8: return launch_ex(c, acoustic3d_stream_kernel<8, true>, a, nb, block, smem, st);
+            default: return (c->opt_dbg & 32) ? launch_ex(c, acoustic3d_stream_kernel<16, false>, a, nb, block, smem, st)
+                                             : launch_ex(c, acoustic3d_stream_kernel<16, true>, a, nb, block, smem, st);
         }
     }
 }

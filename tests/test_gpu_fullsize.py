@@ -1,0 +1,81 @@
+"""-m gpu tests at BASELINE.json's full grid sizes, in the launch configuration bench.py times (time-blocked
+probing, T = 16).  c1 (2D acoustic, 1751x751, nt = 6000, r = 32, 41 offsets) is compared with the oracle element by
+element over the whole shot; c2 (TTI, 2000x800) over a shortened record; c4 (3D, 512x512x256), which the oracle
+cannot finish in seconds, on sampled outputs the oracle can compute (receiver traces of a cropped-in-time run on a
+sub-volume are covered by test_gpu_parity.py) and on properties that hold at any size: gather[h=0] == image bit for
+bit, run-to-run repeatability, and independence of the result from the probe block size T."""
+import numpy as np
+import pytest
+
+import rtm_inputs as ri
+from gpu_util import TOL_FIELD, TOL_IMAGE, rel, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def test_c1_full_shot_against_oracle():
+    """Whole benchmark shot: 6000 steps forward + 6000 adjoint on the full 1911x911 padded grid."""
+    p = ri.make_c3()
+    # reading C19: adjoint input = F(true model) - F(migration model), both computed by the oracle
+    import oracle as orc
+    d_true = orc.forward(p, orc.coeffs(p, vp=p.vp_true))["samples"]
+    co = orc.coeffs(p)
+    f = orc.forward(p, co, Z=p.Z)
+    din = (d_true - f["samples"]).astype(np.float32)
+    a = orc.adjoint(p, co, din, Z=p.Z)
+    img = orc.image(f["PZ"], a["PZ"], 1.0 / p.r)
+    gat = orc.offset_gather(p.n, f["PZ"], a["PZ"], p.offsets, 1.0 / p.r)
+    g = run_gpu(p, din=din, offsets=p.offsets, probe_block=16)
+    errs = {"data": rel(g["data"], f["samples"]), "qadj": rel(g["qadj"], a["samples"]), "Uz": rel(g["Uz"], f["PZ"]),
+            "Vz": rel(g["Vz"], a["PZ"]), "image": rel(g["image"], img), "gather": rel(g["gather"], gat)}
+    print("c1 full", {k: "%.2e" % v for k, v in errs.items()})
+    assert errs["data"] <= TOL_FIELD and errs["qadj"] <= TOL_FIELD, errs
+    for k in ("Uz", "Vz", "image", "gather"):
+        assert errs[k] <= TOL_IMAGE, (k, errs)
+    assert np.array_equal(g["gather"][20], g["image"])          # h = 0 is the zero-offset image, bit for bit
+
+
+def test_c2_full_grid_short_record():
+    p = ri.make_c2()
+    nt = 400
+    p.nt, p.wav, p.Z = nt, np.ascontiguousarray(p.wav[:nt]), np.ascontiguousarray(p.Z[:nt])
+    offs = np.array([-20, 0, 20], np.int32)
+    g = run_gpu(p, offsets=offs, probe_block=16)
+    o = run_oracle(p, g["din"], offsets=offs)
+    errs = {k: rel(g[k], o[k]) for k in ("data", "qadj", "Uz", "Vz", "image", "gather")}
+    print("c2 full grid nt=%d" % nt, {k: "%.2e" % v for k, v in errs.items()})
+    assert errs["data"] <= TOL_FIELD and errs["qadj"] <= TOL_FIELD, errs
+    for k in ("Uz", "Vz", "image", "gather"):
+        assert errs[k] <= TOL_IMAGE, (k, errs)
+
+
+def test_c4_full_grid_properties():
+    """512x512x256 (+40): properties that need no oracle, plus sampled receiver traces against the oracle."""
+    import torch
+    from paper_2201_06914_b200 import Rtm
+    import oracle as orc
+    p = ri.make_c4()
+    nt = 24
+    p.nt, p.wav, p.Z = nt, np.ascontiguousarray(p.wav[:nt]), np.ascontiguousarray(p.Z[:nt])
+    out = {}
+    for T in (16, 0):
+        m = Rtm.from_problem(p, probe_block=T)
+        m.set_model_from_earth(p.vp)
+        m.set_probes(p.Z)
+        data = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+        img, _ = m.adjoint_image(p.rec_xyz, data, p.src_xyz)
+        gat = m.offset_gather(np.array([0, 3], np.int32))
+        torch.cuda.synchronize()
+        out[T] = (data.cpu().numpy(), img.cpu().numpy().ravel(), gat.cpu().numpy().reshape(2, -1))
+        m.close()
+        del m, data, img, gat
+        torch.cuda.empty_cache()
+    d16, i16, g16 = out[16]
+    d0, i0, g0 = out[0]
+    assert np.array_equal(g16[0], i16) and np.array_equal(g0[0], i0)       # gather[h=0] == image
+    assert np.abs(i16).max() > 0 and np.abs(d16).max() > 0
+    # the streaming kernel (T = 16) and the plain kernel (T = 0) are different code paths of the same scheme
+    assert rel(d16, d0) <= TOL_FIELD and rel(i16, i0) <= TOL_IMAGE and rel(g16[1], g0[1]) <= TOL_IMAGE
+    # sampled outputs against the oracle: the forward pass of the full grid for the same 24 steps (about half a minute of CPU)
+    f = orc.forward(p, orc.coeffs(p))
+    assert rel(d16, f["samples"]) <= TOL_FIELD, rel(d16, f["samples"])
