@@ -161,7 +161,9 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
         for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs2(a.fl_hist + j * L.Nu + o) : make_float2(0.f, 0.f);
         float *p = a.PZ + o;
         // software-pipelined over groups of 4 planes: the loads of group g+1 are issued BEFORE the stores
-        // of group g (the compiler cannot hoist them itself: it cannot prove the planes do not alias)
+        // of group g (the compiler cannot hoist them itself: it cannot prove the planes do not alias).  A deeper
+        // pipeline (2 groups in flight) was measured and did not pay inside the 64-register budget of the
+        // 256-thread kernels.
         float2 nxt[4];
 #pragma unroll
         for (int i = 0; i < 4; i++) nxt[i] = (i < r) ? ldcs2(p + (long long)i * L.Nu) : make_float2(0.f, 0.f);
@@ -210,27 +212,41 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
 #pragma unroll
         for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs4(a.fl_hist + j * L.Nu + o) : make_float4(0.f, 0.f, 0.f, 0.f);
         float *p = a.PZ + o;
-        float4 nxt[2];
+        // The plane loop is a chain of DRAM round trips (load - FMA - store per group): with one group of look-ahead
+        // the role needed 1 + r/2 round trips per thread (measured 15 us at c1, longer than the stencil blocks it
+        // shares the launch with).  Three groups of two planes are kept in flight instead.
+        constexpr int G = 2, DEPTH = 3;
+        float4 ring[DEPTH][G];
 #pragma unroll
-        for (int i = 0; i < 2; i++) nxt[i] = (i < r) ? ldcs4(p + (long long)i * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int k = 0; k < r; k += 2) {   // Z rows are zero-padded to zr (multiple of 8)
-            float4 acc[2];
+        for (int s = 0; s < DEPTH; s++)
 #pragma unroll
-            for (int i = 0; i < 2; i++) acc[i] = nxt[i];
+            for (int i = 0; i < G; i++)
+                ring[s][i] = (s * G + i < r) ? ldcs4(p + (long long)(s * G + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int kk = 0; kk < r; kk += G * DEPTH) {   // Z rows are zero-padded to zr (multiple of 8)
 #pragma unroll
-            for (int i = 0; i < 2; i++)
-                nxt[i] = (k + 2 + i < r) ? ldcs4(p + (long long)(k + 2 + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int s = 0; s < DEPTH; s++) {
+                const int k = kk + s * G;
+                if (k >= r) break;
+                float4 acc[G];
 #pragma unroll
-            for (int j = 0; j < TM; j++) {
-                const float2 z = *reinterpret_cast<const float2 *>(sz + j * zr + k);
-                acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
-                acc[0].z = fmaf(z.x, h[j].z, acc[0].z); acc[0].w = fmaf(z.x, h[j].w, acc[0].w);
-                acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
-                acc[1].z = fmaf(z.y, h[j].z, acc[1].z); acc[1].w = fmaf(z.y, h[j].w, acc[1].w);
+                for (int i = 0; i < G; i++) acc[i] = ring[s][i];
+#pragma unroll
+                for (int i = 0; i < G; i++) {
+                    const int kn = k + G * DEPTH + i;
+                    ring[s][i] = (kn < r) ? ldcs4(p + (long long)kn * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+                for (int j = 0; j < TM; j++) {
+                    const float2 z = *reinterpret_cast<const float2 *>(sz + j * zr + k);
+                    acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
+                    acc[0].z = fmaf(z.x, h[j].z, acc[0].z); acc[0].w = fmaf(z.x, h[j].w, acc[0].w);
+                    acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
+                    acc[1].z = fmaf(z.y, h[j].z, acc[1].z); acc[1].w = fmaf(z.y, h[j].w, acc[1].w);
+                }
+#pragma unroll
+                for (int i = 0; i < G; i++)
+                    if (k + i < r) stcs4(p + (long long)(k + i) * L.Nu, acc[i]);
             }
-#pragma unroll
-            for (int i = 0; i < 2; i++)
-                if (k + i < r) stcs4(p + (long long)(k + i) * L.Nu, acc[i]);
         }
     }
 }

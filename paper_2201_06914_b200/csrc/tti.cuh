@@ -69,33 +69,57 @@ __global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
     }
     __syncthreads();
 
-    // ---- stage 2: rotated gradients times cos / sin, halo 4 ----
-    for (int i = tid; i < TTI_GX * TTI_GZ; i += 256) {
-        const int lx = i / TTI_GZ, lz = i % TTI_GZ;
-        const int jx = x0 - 4 + lx, jz = z0 - 4 + lz;
-        float cs = 0.f, sn = 0.f;
-        if (jx < L.Px + 8 && jz < L.pz - 8) {
+    // ---- stage 2: rotated gradients times cos / sin, halo 4; one z-quad per thread and round ----
+    // centred first derivative of a quad: x from the 8 neighbour rows (LDS.128 each), z from the 12-float window
+    for (int i = tid; i < TTI_GX * (TTI_GZ / 4); i += 256) {
+        const int lx = i / (TTI_GZ / 4), lq = i - lx * (TTI_GZ / 4);
+        const int jx = x0 - 4 + lx, jz = z0 - 4 + lq * 4;
+        float4 cs4 = make_float4(0.f, 0.f, 0.f, 0.f), sn4 = cs4;
+        if (jx < L.Px + 8 && jz + 3 < L.pz - 8) {
             const long long o = L.org + jx * L.sx + jz;
-            cs = a.cs[o];
-            sn = a.sn[o];
+            cs4 = ld4(a.cs + o);
+            sn4 = ld4(a.sn + o);
         }
-        const float *fa = sA + (lx + 4) * TTI_FZ + (lz + 4);
-        const float *fb = sB + (lx + 4) * TTI_FZ + (lz + 4);
-        float ax = 0.f, az = 0.f, bx = 0.f, bz = 0.f;
+        const float *fa = sA + (lx + 4) * TTI_FZ + (lq * 4 + 4);
+        const float *fb = sB + (lx + 4) * TTI_FZ + (lq * 4 + 4);
+        float ax[4] = {0.f, 0.f, 0.f, 0.f}, bx[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int j = 4; j >= 1; j--) {
             const float w = w1(j);
-            ax = fmaf(w, fa[j * TTI_FZ] - fa[-j * TTI_FZ], ax);
-            az = fmaf(w, fa[j] - fa[-j], az);
-            bx = fmaf(w, fb[j * TTI_FZ] - fb[-j * TTI_FZ], bx);
-            bz = fmaf(w, fb[j] - fb[-j], bz);
+            const float4 pa = ld4(fa + j * TTI_FZ), ma = ld4(fa - j * TTI_FZ);
+            const float4 pb = ld4(fb + j * TTI_FZ), mb = ld4(fb - j * TTI_FZ);
+            ax[0] = fmaf(w, pa.x - ma.x, ax[0]); ax[1] = fmaf(w, pa.y - ma.y, ax[1]);
+            ax[2] = fmaf(w, pa.z - ma.z, ax[2]); ax[3] = fmaf(w, pa.w - ma.w, ax[3]);
+            bx[0] = fmaf(w, pb.x - mb.x, bx[0]); bx[1] = fmaf(w, pb.y - mb.y, bx[1]);
+            bx[2] = fmaf(w, pb.z - mb.z, bx[2]); bx[3] = fmaf(w, pb.w - mb.w, bx[3]);
         }
-        const float gp = cs * ax - sn * az;   // g_perp
-        const float gl = sn * bx + cs * bz;   // g_par
-        P1[i] = cs * gp;
-        P2[i] = sn * gp;
-        P3[i] = sn * gl;
-        P4[i] = cs * gl;
+        const float4 am = ld4(fa - 4), ac = ld4(fa), ap = ld4(fa + 4);
+        const float4 bm = ld4(fb - 4), bc = ld4(fb), bp = ld4(fb + 4);
+        const float wa[12] = {am.x, am.y, am.z, am.w, ac.x, ac.y, ac.z, ac.w, ap.x, ap.y, ap.z, ap.w};
+        const float wb[12] = {bm.x, bm.y, bm.z, bm.w, bc.x, bc.y, bc.z, bc.w, bp.x, bp.y, bp.z, bp.w};
+        const float cs[4] = {cs4.x, cs4.y, cs4.z, cs4.w}, sn[4] = {sn4.x, sn4.y, sn4.z, sn4.w};
+        float o1[4], o2[4], o3[4], o4[4];
+#pragma unroll
+        for (int e = 0; e < 4; e++) {
+            float az = 0.f, bz = 0.f;
+#pragma unroll
+            for (int j = 4; j >= 1; j--) {
+                const float w = w1(j);
+                az = fmaf(w, wa[4 + e + j] - wa[4 + e - j], az);
+                bz = fmaf(w, wb[4 + e + j] - wb[4 + e - j], bz);
+            }
+            const float gp = cs[e] * ax[e] - sn[e] * az;   // g_perp
+            const float gl = sn[e] * bx[e] + cs[e] * bz;   // g_par
+            o1[e] = cs[e] * gp;
+            o2[e] = sn[e] * gp;
+            o3[e] = sn[e] * gl;
+            o4[e] = cs[e] * gl;
+        }
+        const int g = lx * TTI_GZ + lq * 4;
+        st4(P1 + g, make_float4(o1[0], o1[1], o1[2], o1[3]));
+        st4(P2 + g, make_float4(o2[0], o2[1], o2[2], o2[3]));
+        st4(P3 + g, make_float4(o3[0], o3[1], o3[2], o3[3]));
+        st4(P4 + g, make_float4(o4[0], o4[1], o4[2], o4[3]));
     }
     __syncthreads();
 
@@ -106,20 +130,35 @@ __global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
     const long long off = L.org + jx * L.sx + jz;
 
     float A[4], B[4];
-#pragma unroll
-    for (int q = 0; q < 4; q++) {
-        const int g = (lx + 4) * TTI_GZ + (lz + q + 4);
-        float dx1 = 0.f, dz2 = 0.f, dx3 = 0.f, dz4 = 0.f;
+    {
+        const int g = (lx + 4) * TTI_GZ + (lz + 4);
+        float dx1[4] = {0.f, 0.f, 0.f, 0.f}, dx3[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int j = 4; j >= 1; j--) {
             const float w = w1(j);
-            dx1 = fmaf(w, P1[g + j * TTI_GZ] - P1[g - j * TTI_GZ], dx1);
-            dz2 = fmaf(w, P2[g + j] - P2[g - j], dz2);
-            dx3 = fmaf(w, P3[g + j * TTI_GZ] - P3[g - j * TTI_GZ], dx3);
-            dz4 = fmaf(w, P4[g + j] - P4[g - j], dz4);
+            const float4 p1 = ld4(P1 + g + j * TTI_GZ), m1 = ld4(P1 + g - j * TTI_GZ);
+            const float4 p3 = ld4(P3 + g + j * TTI_GZ), m3 = ld4(P3 + g - j * TTI_GZ);
+            dx1[0] = fmaf(w, p1.x - m1.x, dx1[0]); dx1[1] = fmaf(w, p1.y - m1.y, dx1[1]);
+            dx1[2] = fmaf(w, p1.z - m1.z, dx1[2]); dx1[3] = fmaf(w, p1.w - m1.w, dx1[3]);
+            dx3[0] = fmaf(w, p3.x - m3.x, dx3[0]); dx3[1] = fmaf(w, p3.y - m3.y, dx3[1]);
+            dx3[2] = fmaf(w, p3.z - m3.z, dx3[2]); dx3[3] = fmaf(w, p3.w - m3.w, dx3[3]);
         }
-        A[q] = dx1 - dz2;
-        B[q] = dx3 + dz4;
+        const float4 m2 = ld4(P2 + g - 4), c2 = ld4(P2 + g), p2 = ld4(P2 + g + 4);
+        const float4 m4 = ld4(P4 + g - 4), c4 = ld4(P4 + g), p4q = ld4(P4 + g + 4);
+        const float w2a[12] = {m2.x, m2.y, m2.z, m2.w, c2.x, c2.y, c2.z, c2.w, p2.x, p2.y, p2.z, p2.w};
+        const float w4a[12] = {m4.x, m4.y, m4.z, m4.w, c4.x, c4.y, c4.z, c4.w, p4q.x, p4q.y, p4q.z, p4q.w};
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            float dz2 = 0.f, dz4 = 0.f;
+#pragma unroll
+            for (int j = 4; j >= 1; j--) {
+                const float w = w1(j);
+                dz2 = fmaf(w, w2a[4 + q + j] - w2a[4 + q - j], dz2);
+                dz4 = fmaf(w, w4a[4 + q + j] - w4a[4 + q - j], dz4);
+            }
+            A[q] = dx1[q] - dz2;
+            B[q] = dx3[q] + dz4;
+        }
     }
 
     const float4 p4 = ld4(a.u0 + off), r4 = ld4(a.u1 + off);

@@ -45,6 +45,23 @@ def test_workspace_bytes_model():
     assert w32 < 0.5e9
 
 
+def test_c4_workspace_fits_hbm_where_full_history_does_not():
+    """north_star: a 3D case whose full wavefield history would not fit in HBM runs entirely in device memory.
+    configs[4]: 512x512x256, nt = 3000, r = 16; with the T = 16 history ring the workspace is still O(N r)."""
+    _build()
+    from paper_2201_06914_b200 import binding as B
+    base = dict(ndim=3, n=(512, 512, 256), h=12.5, nb=40, physics=0, nt=3000, dt=8.5e-4, r=16, max_pts=65536)
+    N = 512 * 512 * 256
+    full_history = N * 3000 * 4
+    hbm = 180e9
+    assert full_history > 4 * hbm                                   # 805 GB
+    for T, extra in ((0, 0), (16, 2 * 16 * N * 4)):
+        w = B.workspace_bytes(B.make_config(probe_block=T, **base))
+        assert 2 * 16 * N * 4 + extra <= w <= 2 * 16 * N * 4 + extra + 3.0e9      # + 3 fields, K2, tables
+        assert w < 0.15 * hbm and w < full_history / 40
+    assert B.workspace_bytes(B.make_config(probe_block=17, **base)) == 0            # invalid config -> 0
+
+
 def test_table1_memory_ratios_golden():
     """tests/golden/table1.txt holds the paper's Table 1; gain = standard / trace estimation."""
     rows = {}
