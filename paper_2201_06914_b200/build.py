@@ -8,13 +8,20 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "librtm.so")
 SOURCES = ["rtm.cu"]
-DEPS = ["rtm.cu", "common.cuh", "acoustic.cuh", "tti.cuh", "image.cuh", os.path.join("..", "..", "include", "rtm.h")]
+
+
+def _deps():
+    """Every source the library is built from: all of csrc/*.cu, csrc/*.cuh and the public header."""
+    import glob
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))) + [
+        os.path.join(HERE, "..", "include", "rtm.h")]
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    newest = max(os.path.getmtime(os.path.join(CSRC, d)) for d in DEPS)
+    newest = max(os.path.getmtime(d) for d in _deps())
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp.%d" % os.getpid()

@@ -25,8 +25,8 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
     extern __shared__ __align__(16) float dyn_smem[];
     const Layout &L = a.L;
     const int tid = threadIdx.x;
-    pdl_launch_dependents();
     if (blockIdx.x < (unsigned)a.fl_blocks) {
+        pdl_launch_dependents();
         flush_role4<TM>(a, dyn_smem, tid, 128, blockIdx.x);
         return;
     }
@@ -108,6 +108,9 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
     const bool zdamp = (dzv[0] != 0.f) | (dzv[1] != 0.f) | (dzv[2] != 0.f) | (dzv[3] != 0.f);
 
     pdl_wait();   // from here on the previous step's fields are complete and visible
+    // Dependents are released only now: a block of step n+1 can therefore only start once step n-1 is complete,
+    // which is what lets the flush role of step n+1 skip its own wait (see flush_role4) and overlap with step n.
+    pdl_launch_dependents();
 
     const float *__restrict__ u0 = a.u0;
     const float *__restrict__ K2 = a.K2;
@@ -169,39 +172,52 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
         }
         if (!valid) continue;
         const float cc[4] = {c.x, c.y, c.z, c.w};
-        float lap[4] = {0.f, 0.f, 0.f, 0.f};
+        // Laplacian in the difference form, two z points per instruction (FADD2 / FFMA2); the same operations in the
+        // same order per point as the scalar kernels: s = (z part + x part), lap = fma(w, s, lap), small weights first
+        const f32x2 clo = pk(c.x, c.y), chi = pk(c.z, c.w);
+        f32x2 llo = pk(0.f, 0.f), lhi = llo;
 #pragma unroll
-        for (int j = 4; j >= 1; j--) {   // small weights first
+        for (int j = 4; j >= 1; j--) {
             const float4 P = q[4 + rr + j], M = q[4 + rr - j];
-            const float xs[4] = {(P.x - c.x) + (M.x - c.x), (P.y - c.y) + (M.y - c.y),
-                                 (P.z - c.z) + (M.z - c.z), (P.w - c.w) + (M.w - c.w)};
+            const f32x2 xlo = dd2(pk(P.x, P.y), pk(M.x, M.y), clo), xhi = dd2(pk(P.z, P.w), pk(M.z, M.w), chi);
+            f32x2 zlo, zhi;
+            if (j % 2 == 0) {   // shifted z windows are register-pair aligned for even shifts only
+                zlo = dd2(pk(win[4 + j], win[5 + j]), pk(win[4 - j], win[5 - j]), clo);
+                zhi = dd2(pk(win[6 + j], win[7 + j]), pk(win[6 - j], win[7 - j]), chi);
+            } else {
+                float zs[4];
+#pragma unroll
+                for (int e = 0; e < 4; e++) zs[e] = (win[4 + e + j] - cc[e]) + (win[4 + e - j] - cc[e]);
+                zlo = pk(zs[0], zs[1]);
+                zhi = pk(zs[2], zs[3]);
+            }
             const float w = w2(j);
-#pragma unroll
-            for (int e = 0; e < 4; e++) {
-                const float s = ((win[4 + e + j] - cc[e]) + (win[4 + e - j] - cc[e])) + xs[e];
-                lap[e] = fmaf(w, s, lap[e]);
-            }
+            const f32x2 ww = pk(w, w);
+            llo = fma2(ww, add2(zlo, xlo), llo);
+            lhi = fma2(ww, add2(zhi, xhi), lhi);
         }
-        float d[4];
+        const f32x2 k2lo = pk(k2[0], k2[1]), k2hi = pk(k2[2], k2[3]);
+        const f32x2 dulo = pk(du[0], du[1]), duhi = pk(du[2], du[3]);
+        f32x2 dlo, dhi;
         if (sxc == 0.f && !zdamp) {
-#pragma unroll
-            for (int e = 0; e < 4; e++) d[e] = fmaf(k2[e], lap[e], du[e]);          // K1 = 1 exactly
+            dlo = fma2(k2lo, llo, dulo);          // K1 = 1 exactly
+            dhi = fma2(k2hi, lhi, duhi);
         } else {
+            float k1[4];
 #pragma unroll
-            for (int e = 0; e < 4; e++) {
-                const float k1 = sxc == 0.f ? k1z[e] : (dzv[e] == 0.f ? k1xc : k1_of(sxc + dzv[e]));
-                d[e] = fmaf(k1, du[e], k2[e] * lap[e]);
-            }
+            for (int e = 0; e < 4; e++) k1[e] = sxc == 0.f ? k1z[e] : (dzv[e] == 0.f ? k1xc : k1_of(sxc + dzv[e]));
+            dlo = fma2(pk(k1[0], k1[1]), dulo, mul2(k2lo, llo));
+            dhi = fma2(pk(k1[2], k1[3]), duhi, mul2(k2hi, lhi));
         }
         if (imask & (1u << rr)) {   // a3: K2 * scale * w * val
             const float4 iv = injs[rr * 128 + tid];
-            d[0] = fmaf(k2[0], iv.x, d[0]);
-            d[1] = fmaf(k2[1], iv.y, d[1]);
-            d[2] = fmaf(k2[2], iv.z, d[2]);
-            d[3] = fmaf(k2[3], iv.w, d[3]);
+            dlo = fma2(k2lo, pk(iv.x, iv.y), dlo);
+            dhi = fma2(k2hi, pk(iv.z, iv.w), dhi);
         }
-        float4 dn = make_float4(d[0], d[1], d[2], d[3]);
-        float4 un = make_float4(cc[0] + d[0], cc[1] + d[1], cc[2] + d[2], cc[3] + d[3]);
+        const f32x2 ulo = add2(clo, dlo), uhi = add2(chi, dhi);
+        float4 dn, un;
+        upk(dlo, dn.x, dn.y); upk(dhi, dn.z, dn.w);
+        upk(ulo, un.x, un.y); upk(uhi, un.z, un.w);
         if (!full) {   // ragged quad at the end of a row: keep the halo zero
             if (jz + 1 >= L.Pz) { dn.y = 0.f; un.y = 0.f; }
             if (jz + 2 >= L.Pz) { dn.z = 0.f; un.z = 0.f; }

@@ -69,8 +69,8 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     extern __shared__ __align__(16) float dyn_smem[];
     const Layout &L = a.L;
     const int tid = threadIdx.x;
-    pdl_launch_dependents();
     if (blockIdx.x < (unsigned)a.fl_blocks) {
+        pdl_launch_dependents();
         flush_role<TM>(a, dyn_smem, tid, 256, blockIdx.x);
         return;
     }
@@ -117,6 +117,7 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     const bool zdamp = (dzv[0] != 0.f) | (dzv[1] != 0.f) | (dzv[2] != 0.f) | (dzv[3] != 0.f);
 
     pdl_wait();   // from here on the previous step's fields are complete and visible
+    pdl_launch_dependents();   // only now: lets the next step's flush role run without a wait (see flush_role)
     sample_points(a, lin_block, 256, tid);
 
     const float *__restrict__ u0 = a.u0;

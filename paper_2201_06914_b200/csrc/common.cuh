@@ -61,6 +61,7 @@ struct StepArgs {
     long long fl_zstep;     // +zr forward, -zr adjoint
     int fl_n;               // slots in that block
     int fl_blocks;
+    int fl_nowait;          // the flush role may skip griddepcontrol.wait (its inputs are >= 2 launches old)
     long long fl_q0, fl_q1;   // slice of this launch in units of float2 (flush_role) or float4 (flush_role4)
     int zr;
     unsigned gx, gy;        // stencil grid extents (the launch grid is 1-D: fl_blocks + gx*gy*gz)
@@ -149,7 +150,11 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
         sz[i] = j < n ? a.fl_Z0[j * a.fl_zstep + k] : 0.0f;
     }
     __syncthreads();
-    pdl_wait();   // the Z rows above are static; the history was written by earlier launches
+    // The history being flushed was written at least two launches ago whenever fl_nowait is set (the host schedules
+    // the slices on slots >= 1 of the time block) and the stencil blocks release their dependents only after their
+    // own wait, so every launch <= n-2 is complete when a block of launch n runs: no wait needed, and the role
+    // overlaps with the previous step instead of starting behind it.
+    if (!a.fl_nowait) pdl_wait();
     const int np = L.upz / 2;
     for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
         const long long row = t / np;
@@ -201,7 +206,7 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
         sz[i] = j < n ? a.fl_Z0[j * a.fl_zstep + k] : 0.0f;
     }
     __syncthreads();
-    pdl_wait();
+    if (!a.fl_nowait) pdl_wait();   // see flush_role
     const int nq = L.upz / 4;
     for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
         const long long row = t / nq;

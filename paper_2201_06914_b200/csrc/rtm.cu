@@ -511,8 +511,8 @@ static step_fn stream2d_fn(int rx) {
     return rx <= 2 ? acoustic2d_stream_kernel<TM, 2> : rx <= 4 ? acoustic2d_stream_kernel<TM, 4>
          : rx <= 8 ? acoustic2d_stream_kernel<TM, 8> : acoustic2d_stream_kernel<TM, 16>;
 }
-// Rows per thread of the 2D streaming kernel: the smallest RX in {2,4,8,16} whose grid fits in one wave
-// of resident blocks (most parallelism without a second, nearly empty wave); large problems use 8.
+// Rows per thread of the 2D streaming kernel: the smallest RX in {2,4,8,16} whose launch (stencil + flush blocks) fits
+// in two waves of resident blocks; larger problems use 4.
 static int pick_rx(rtm_ctx *c) {
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
@@ -520,16 +520,19 @@ static int pick_rx(rtm_ctx *c) {
     const int tm = tm_of(c->T);
     // flush-role blocks that share every launch: one float4 of the physical grid per thread, 1/T of it per step
     const long long quads = (long long)c->L.nx * c->L.ny * (c->L.upz / 4);
-    const long long fblocks = (quads / std::max(1, c->T) + 127) / 128 + 1;
+    const long long fblocks = (quads / std::max(1, c->T - 1) + 127) / 128 + 1;
     const int cand[4] = {2, 4, 8, 16};
     for (int i = 0; i < 4; i++) {
         step_fn f = tm <= 4 ? stream2d_fn<4>(cand[i]) : tm <= 8 ? stream2d_fn<8>(cand[i]) : stream2d_fn<16>(cand[i]);
         int per_sm = 0;
         cudaFuncSetAttribute((const void *)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, 128, stream_smem(c, cand[i])) != cudaSuccess) { cudaGetLastError(); continue; }
-        if (stream_blocks(c, cand[i]) + fblocks <= (long long)per_sm * nsm) return cand[i];
+        // measured at c1 (1911 x 911, T = 16): RX = 4 (1028 blocks, 1.7 waves) 12.4 us per step, RX = 8 (591 blocks, one
+        // wave) 13.5 us, RX = 16 15.9 us: fine-grained blocks balance the stencil and flush roles better than one
+        // wave of long-lived ones, as long as the launch stays within two waves
+        if (stream_blocks(c, cand[i]) + fblocks <= 2LL * per_sm * nsm) return cand[i];
     }
-    return 8;
+    return 4;
 }
 
 static int tm_of(int T) { return T <= 0 ? 0 : T <= 4 ? 4 : T <= 8 ? 8 : 16; }
@@ -670,9 +673,15 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
                 a.fl_hist = c->hist + (size_t)(pb & 1) * T * L.Nu;
                 a.fl_Z0 = Z + (size_t)nfirst * c->zr;
                 a.fl_n = T;
-                a.fl_q0 = units * slot / len_b;
-                a.fl_q1 = units * (slot + 1) / len_b;
-                a.fl_blocks = (int)((a.fl_q1 - a.fl_q0 + bthreads - 1) / bthreads);   // one unit per thread
+                // slices go to slots 1 .. len_b-1: their input (the previous block's last slot) is then at least two
+                // launches old and the role needs no grid dependency; a block of one step flushes on slot 0, waiting
+                const int nsl = len_b > 1 ? len_b - 1 : 1, sl = len_b > 1 ? slot - 1 : 0;
+                a.fl_nowait = (len_b > 1 && c->opt_pdl) ? 1 : 0;
+                if (sl >= 0) {
+                    a.fl_q0 = units * sl / nsl;
+                    a.fl_q1 = units * (sl + 1) / nsl;
+                    a.fl_blocks = (int)((a.fl_q1 - a.fl_q0 + bthreads - 1) / bthreads);   // one unit per thread
+                }
             }
         }
         if ((c->opt_dbg & 3) == 1) a.fl_blocks = 0;

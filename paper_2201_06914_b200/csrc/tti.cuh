@@ -32,14 +32,16 @@ __global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
     float *P3 = P2 + TTI_GX * TTI_GZ;          // sin g_par
     float *P4 = P3 + TTI_GX * TTI_GZ;          // cos g_par
 
-    pdl_launch_dependents();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 16 + threadIdx.x;
+    if (TM == 0) pdl_launch_dependents();
     if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
+        pdl_launch_dependents();
         flush_role<(TM > 0 ? TM : 1)>(a, smem, tid, 256, blockIdx.x);
         return;
     }
     pdl_wait();
+    if (TM > 0) pdl_launch_dependents();   // only now: lets the next step's flush role run without a wait (see flush_role)
     const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
     sample_points(a, lin_block, 256, tid);
 
