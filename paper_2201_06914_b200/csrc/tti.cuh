@@ -123,13 +123,23 @@ __global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
         st4(P3 + g, make_float4(o3[0], o3[1], o3[2], o3[3]));
         st4(P4 + g, make_float4(o4[0], o4[1], o4[2], o4[3]));
     }
+    // stage-3 operands are requested BEFORE the barrier, so that their L2 latency overlaps with the barrier wait
+    // and the shared-memory arithmetic of stage 3 instead of sitting in front of the update
+    const int lx = threadIdx.y, lz = threadIdx.x * 4;
+    const int jx = x0 + lx, jz = z0 + lz;
+    const bool act3 = jx < L.Px && jz < L.Pz;
+    const long long off = L.org + jx * L.sx + jz;
+    float4 p4 = make_float4(0.f, 0.f, 0.f, 0.f), r4 = p4, dp4 = p4, dr4 = p4, k24 = p4, e4 = p4, d4 = p4;
+    if (act3) {
+        p4 = ld4(a.u0 + off); r4 = ld4(a.u1 + off);
+        dp4 = ld4(a.d0 + off); dr4 = ld4(a.d1 + off);
+        k24 = ld4(a.K2 + off);
+        if (!a.adjoint) { e4 = ld4(a.epsh + off); d4 = ld4(a.delh + off); }
+    }
     __syncthreads();
 
     // ---- stage 3: second derivative pass, update, inject, probe ----
-    const int lx = threadIdx.y, lz = threadIdx.x * 4;
-    const int jx = x0 + lx, jz = z0 + lz;
-    if (jx >= L.Px || jz >= L.Pz) return;
-    const long long off = L.org + jx * L.sx + jz;
+    if (!act3) return;
 
     float A[4], B[4];
     {
@@ -163,15 +173,11 @@ __global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
         }
     }
 
-    const float4 p4 = ld4(a.u0 + off), r4 = ld4(a.u1 + off);
-    const float4 dp4 = ld4(a.d0 + off), dr4 = ld4(a.d1 + off);
-    const float4 k24 = ld4(a.K2 + off);
     const float pc[4] = {p4.x, p4.y, p4.z, p4.w}, rc[4] = {r4.x, r4.y, r4.z, r4.w};
     const float dp[4] = {dp4.x, dp4.y, dp4.z, dp4.w}, dr[4] = {dr4.x, dr4.y, dr4.z, dr4.w};
     const float k2[4] = {k24.x, k24.y, k24.z, k24.w};
     float eh[4] = {1.f, 1.f, 1.f, 1.f}, dh[4] = {0.f, 0.f, 0.f, 0.f};
     if (!a.adjoint) {
-        const float4 e4 = ld4(a.epsh + off), d4 = ld4(a.delh + off);
         eh[0] = e4.x; eh[1] = e4.y; eh[2] = e4.z; eh[3] = e4.w;
         dh[0] = d4.x; dh[1] = d4.y; dh[2] = d4.z; dh[3] = d4.w;
     }
