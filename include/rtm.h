@@ -47,7 +47,8 @@ typedef struct {
     int probe_block;/* T_b: 0|1 = probe fused into every time step (8 r bytes/point/step of Uz traffic);
                        2..16 = time-blocked probing: each step stores its field into a T_b-slot history
                        ring and every T_b steps one flush applies T_b rows of Z (traffic / T_b).
-                       Same sums, same order per (k,x); costs T_b N floats of workspace.           */
+                       Same sums, same order per (k,x); costs 2 T_b N floats of workspace (the ring is
+                       double-buffered: one half is filled while the other is flushed).             */
 } rtm_config;
 
 /* Bytes of device workspace rtm_create needs for this config; 0 if the config is invalid.
@@ -137,7 +138,14 @@ float rtm_last_pass_ms(rtm_ctx *ctx, int which);
 /* Timing experiments (option "dbg" & 16): the first 8 phase time stamps (ns, %globaltimer) of each of the first
  * nblocks (<= 1024) blocks of the last step launch -> h_out [nblocks][8] (HOST).  Synchronises the device.  */
 int rtm_debug_stamps(rtm_ctx *ctx, unsigned long long *h_out, int nblocks);
-/* Tuning knob: name/value pairs: "time_steps" (0|1), "graph" (0|1).      */
+/* Tuning knobs and timing experiments; none of them changes what is computed:
+ *   "time_steps" 0|1  record CUDA events around the step launches of each pass (rtm_last_pass_ms);
+ *   "pdl"        0|1  programmatic dependent launch between consecutive step kernels (default 1);
+ *   "rx"         2|4|8|16|0  rows per thread of the 2D streaming kernel (0 = automatic; T > 1, 2D acoustic only);
+ *   "dbg"        bit mask for timing experiments ONLY (results become wrong): 1 no flush role, 2 no stencil role,
+ *                16 write phase time stamps (rtm_debug_stamps), 32 scalar arithmetic in the 3D streaming kernel
+ *                (this one keeps the results bit-identical).
+ * Errors: RTM_EINVAL (unknown name / value out of range).                                              */
 int rtm_set_option(rtm_ctx *ctx, const char *name, int value);
 
 const char *rtm_strerror(int code);

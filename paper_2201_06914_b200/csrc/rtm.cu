@@ -70,7 +70,7 @@ struct rtm_ctx {
     std::vector<int> snap_steps;
     float *snap_out;
     long long launches;
-    int opt_graph, opt_time, opt_pdl, opt_dbg;
+    int opt_time, opt_pdl, opt_dbg;
     cudaEvent_t ev[2][2];
     bool ev_valid[2];
 };
@@ -216,7 +216,6 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     c->have_model = c->have_probes = c->have_U = c->have_V = false;
     c->snap_out = nullptr;
     c->launches = 0;
-    c->opt_graph = 0;
     c->opt_time = 0;
     c->opt_pdl = 1;
     c->opt_dbg = 0;
@@ -877,7 +876,6 @@ extern "C" long long rtm_launch_count(const rtm_ctx *c) { return c ? c->launches
 
 extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!c || !name) return RTM_EINVAL;
-    if (!strcmp(name, "graph")) { c->opt_graph = value; return RTM_OK; }
     if (!strcmp(name, "time_steps")) { c->opt_time = value; return RTM_OK; }
     if (!strcmp(name, "pdl")) { c->opt_pdl = value; return RTM_OK; }
     if (!strcmp(name, "dbg")) { c->opt_dbg = value; return RTM_OK; }   // timing experiments only: 1 = no flush role, 2 = no stencil
