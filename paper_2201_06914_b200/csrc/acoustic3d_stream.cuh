@@ -37,16 +37,6 @@ constexpr int S3_INJCAP = 512;          // injection amounts (float4) a block ca
 constexpr int S3_SMEM = (S3_NU * S3_TILE + 2 * S3_NK * S3_CT) * 4 + S3_INJCAP * 16;
 static_assert(S3_NU == 5 + S3_D && S3_NK == S3_D + 1, "ring sizes follow the prefetch distance");
 
-// 16-byte asynchronous copy global -> shared; ok == false writes zeros (the source is not read)
-__device__ __forceinline__ void cp_async16(float *dst_smem, const float *src, bool ok) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    const int n = ok ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(n) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 // sum of the injection entries of padded row `row` that fall into the z-quad starting at jz (a3)
 __device__ __forceinline__ float4 inject_lookup(const StepArgs &a, long long row, int jz) {
     float acc[4] = {0.f, 0.f, 0.f, 0.f};

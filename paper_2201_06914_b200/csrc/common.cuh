@@ -131,6 +131,16 @@ template <> struct V2<false> {
     static __device__ __forceinline__ T dd(T P, T M, T c) { return add(sub(P, c), sub(M, c)); }
 };
 
+// 16-byte asynchronous copy global -> shared; ok == false writes zeros (the source is not read)
+__device__ __forceinline__ void cp_async16(float *dst_smem, const float *src, bool ok) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    const int n = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // Programmatic dependent launch: let the next step's grid become resident while this one drains, and
 // wait for the previous grid (and its memory) before touching anything it wrote.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }

@@ -66,6 +66,83 @@ __global__ void __launch_bounds__(256) gather_kernel(Layout L, const float *__re
     }
 }
 
+// a8, register-tiled fast path for a run of consecutive offsets h0, h0+1, ..., h0+nh-1 (nh <= GT_HP).
+//
+// The generic kernel above reads 2 x LDG.128 per 4 FMA and is bound by L1/L2 throughput (c3: 1.39 ms for a 552 MB
+// minimum).  Here a block owns GT_X consecutive x and 32 consecutive floats of the fast axes (z, or (y,z) in 3D: a
+// shift by h along x is a shift by whole rows of R = ny*upz floats) and all offsets; a thread owns an 8 (x) by 8 (h)
+// patch of outputs of one lane.  Per probe k the block stages the GT_X + GT_HP - 1 rows of U and of V it needs in
+// shared memory (cp.async, double-buffered, zero-filled outside [0, nx): Eq. 4's terms vanish there, reading C11);
+// a thread then reads 15 + 15 values and does 64 FMAs: acc[i][j] += U[i + j] * V[i - j + 7].
+// Same products in the same order (k ascending, one fma each) as the generic kernel and as image_kernel, so
+// gather[h = 0] stays bit-identical to the image.
+constexpr int GT_X = 32, GT_HP = 48, GT_ROWS = GT_X + GT_HP - 1, GT_THREADS = 32 * (GT_X / 8) * (GT_HP / 8);
+constexpr int GT_SMEM = 2 * 2 * GT_ROWS * 32 * 4;
+
+__global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, const float *__restrict__ U,
+                                                                   const float *__restrict__ V, int r, int nh, int h0,
+                                                                   float scale, float *__restrict__ G) {
+    extern __shared__ __align__(16) float gsm[];   // [2 buffers][U | V][GT_ROWS][32]
+    const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
+    const int xg = grp % (GT_X / 8), hg = grp / (GT_X / 8);
+    const long long R = (long long)L.ny * L.upz;
+    const long long l0 = (long long)blockIdx.x * 32;          // first float of the fast axes
+    const int x0 = blockIdx.y * GT_X;
+    const int xu0 = x0 + h0, xv0 = x0 - (h0 + GT_HP - 1);     // first x row of the U / V tile
+
+    auto request = [&](int k, int buf) {
+        float *dst = gsm + buf * (2 * GT_ROWS * 32);
+        // 2 * GT_ROWS rows of 128 bytes = 8 chunks of 16 bytes each
+        for (int c = tid; c < 2 * GT_ROWS * 8; c += GT_THREADS) {
+            const int row = c >> 3, q = c & 7;
+            const bool isV = row >= GT_ROWS;
+            const int x = isV ? xv0 + (row - GT_ROWS) : xu0 + row;
+            const bool ok = x >= 0 && x < L.nx;
+            const float *src = (isV ? V : U) + (long long)k * L.Nu + (long long)(ok ? x : 0) * R + l0 + q * 4;
+            cp_async16(dst + row * 32 + q * 4, src, ok);
+        }
+        cp_async_commit();
+    };
+
+    float acc[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+#pragma unroll
+        for (int j = 0; j < 8; j++) acc[i][j] = 0.f;
+
+    request(0, 0);
+    for (int k = 0; k < r; k++) {
+        cp_async_wait<0>();
+        __syncthreads();            // probe k has landed for everybody; nobody still reads the other buffer
+        if (k + 1 < r) request(k + 1, (k + 1) & 1);
+        const float *us = gsm + (k & 1) * (2 * GT_ROWS * 32) + (8 * (xg + hg)) * 32 + lane;
+        const float *vs = gsm + (k & 1) * (2 * GT_ROWS * 32) + (GT_ROWS + 8 * xg - 8 * hg + GT_HP - 8) * 32 + lane;
+        float u[15], v[15];
+#pragma unroll
+        for (int m = 0; m < 15; m++) { u[m] = us[m * 32]; v[m] = vs[m * 32]; }
+#pragma unroll
+        for (int i = 0; i < 8; i++)
+#pragma unroll
+            for (int j = 0; j < 8; j++) acc[i][j] = fmaf(u[i + j], v[i - j + 7], acc[i][j]);
+    }
+
+    // canonical output [nh][nx][ny][nz]: lane -> (iy, iz) of the pitch-padded fast axes
+    const long long l = l0 + lane;
+    const int iy = (int)(l / L.upz), iz = (int)(l - (long long)iy * L.upz);
+    if (iz >= L.nz || iy >= L.ny) return;
+    const long long N = (long long)L.nx * L.ny * L.nz;
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+        const int x = x0 + xg * 8 + i;
+        if (x >= L.nx) break;
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+            const int ih = hg * 8 + j;
+            if (ih < nh) G[(long long)ih * N + ((long long)x * L.ny + iy) * L.nz + iz] = scale * acc[i][j];
+        }
+    }
+}
+
 // canonical [Np] -> internal haloed/pitched layout (halo untouched: it is zeroed once at create)
 __global__ void pack_field_kernel(Layout L, const float *__restrict__ src, float *__restrict__ dst) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -772,8 +772,15 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
     CU(cudaEventRecord(c->offs_done, st));
     c->offs_pending = true;
     const Layout &L = c->L;
-    const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
-    gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, c->offs, scale, d_gather);
+    bool run = nh >= 8 && nh <= GT_HP;   // a run of consecutive offsets takes the register-tiled kernel
+    for (int i = 1; i < nh && run; i++) run = h_offsets[i] == h_offsets[i - 1] + 1;
+    if (run) {
+        const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
+        gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, h_offsets[0], scale, d_gather);
+    } else {
+        const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
+        gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, c->offs, scale, d_gather);
+    }
     c->launches++;
     CU(cudaGetLastError());
     return RTM_OK;

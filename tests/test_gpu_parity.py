@@ -69,6 +69,22 @@ def test_c4_cropped():
     check_all(p, snap_steps=[50, 199])
 
 
+@pytest.mark.parametrize("nd,n,nh", [(2, (45, 70), 9), (2, (130, 257), 48), (3, (21, 9, 37), 13), (2, (30, 33), 41)])
+def test_gather_tiled_path(nd, n, nh):
+    """A run of 8..48 consecutive offsets takes gather_tiled_kernel (ragged x tiles, offsets wider than the grid
+    edge distance, 3D rows of ny*upz floats); other lists take the generic kernel: both against the oracle, and
+    against each other where they overlap."""
+    p = ri.random_acoustic(nd, n=n, nb=4, nt=160, r=5, seed=21, nsrc=1, nrec=6)
+    h0 = -(nh // 2)
+    offs = np.arange(h0, h0 + nh, dtype=np.int32)
+    offs = offs[np.abs(offs) < n[0]]
+    g, o, e = check_all(p, offsets=offs)
+    i0 = int(np.where(offs == 0)[0][0])
+    assert np.array_equal(g["gather"][i0], g["image"])                 # PAPER.md:L52, bit for bit
+    g2 = run_gpu(p, offsets=offs[::2])                                 # stride 2: generic kernel
+    assert np.array_equal(g2["gather"], g["gather"][::2])
+
+
 def test_gather_h0_equals_image_bitwise():
     p = ri.random_acoustic(2, n=(50, 45), nb=8, nt=60, r=6, seed=9)
     g = run_gpu(p, offsets=np.array([0], np.int32))
