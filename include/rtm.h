@@ -82,6 +82,13 @@ int rtm_set_model(rtm_ctx *ctx, const float *d_K2, const float *d_epsh, const fl
  * differencing Z, reading C4).  Copied into the workspace.                                        */
 int rtm_set_probes(rtm_ctx *ctx, const float *d_Zf, const float *d_Za, void *cuda_stream);
 
+/* Host helper for Eq. 2-3's gradient-type imaging condition  sum_t u_tt(t) v(t)  (reading C4):
+ * with w[n] the field computed by step n,  sum_n z[n] (w[n] - 2 w[n-1] + w[n-2]) / dt^2  =  sum_n Zdd[n] w[n],
+ *   Zdd[n][k] = (Z[n][k] - 2 Z[n+1][k] + Z[n+2][k]) / dt^2,   Z[nt] = Z[nt+1] = 0,
+ * so probing u_tt costs nothing: pass Zdd as d_Zf and Z as d_Za to rtm_set_probes.  fp64 arithmetic, one rounding
+ * to fp32.  h_Z, h_Zdd: HOST arrays [nt][r] (may not alias).  Errors: RTM_EINVAL.                      */
+int rtm_probes_dtt_host(int nt, int r, double dt, const float *h_Z, float *h_Zdd);
+
 /* Forward pass with fused probing (Eq. 3: u_bar = Z^T u accumulated on the fly).
  * Zeroes the wavefields and Uz, runs n = 0..nt-1:  time step with fused damping; inject
  * K2 h^(2-d) w wav[n][s] at the 2^d corners of each source; record d[n][j] = sum_c w u[corner];

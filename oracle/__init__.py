@@ -3,6 +3,9 @@
 Thin ctypes wrapper around ``oracle/rtm_oracle.c`` (plain C, fp64, OpenMP over the outer spatial
 loop).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s cpu_baseline /
 ``--impl reference`` legs may import this package.  It imports nothing from the CUDA package.
+
+Beside the C routines it holds two plain numpy functions for Eq. 2-3's gradient-type imaging condition
+(``probes_dtt``, ``exact_gradient_image``; pins in tests/test_oracle_estimator.py).
 """
 from __future__ import annotations
 
@@ -154,6 +157,30 @@ def exact_image(uh, vh):
     vh = np.ascontiguousarray(vh, np.float64)
     I = np.zeros(N, np.float64)
     lib.orc_exact_image(C.c_int(nt), C.c_long(N), _fp(uh), _fp(vh), _fp(I))
+    return I
+
+
+def probes_dtt(Z, dt):
+    """Reading C4 (Eq. 2-3 probe u_tt): Zdd[n] = (Z[n] - 2 Z[n+1] + Z[n+2]) / dt^2 with
+    Z[nt] = Z[nt+1] = 0, so that  sum_n Z[n] (w[n] - 2 w[n-1] + w[n-2]) / dt^2 = sum_n Zdd[n] w[n]  for the fields
+    w[n] computed by step n (w[-1] = w[-2] = 0).  fp64, one rounding to the fp32 the GPU receives (C18)."""
+    Z = np.asarray(Z, np.float32).astype(np.float64)
+    nt = Z.shape[0]
+    Zp = np.vstack([Z, np.zeros((2, Z.shape[1]))])
+    return (((Zp[:nt] - 2.0 * Zp[1:nt + 1]) + Zp[2:nt + 2]) * (1.0 / (float(dt) * float(dt)))).astype(np.float32)
+
+
+def exact_gradient_image(uh, vh, dt):
+    """Eq. 2 as printed: sum_t u_tt(t) v(t) from stored histories [nt][N], with the second time
+    difference of the update itself, u_tt[n] = (w[n] - 2 w[n-1] + w[n-2]) / dt^2 (zero initial fields)."""
+    uh = np.asarray(uh, np.float64)
+    vh = np.asarray(vh, np.float64)
+    nt = uh.shape[0]
+    I = np.zeros(uh.shape[1], np.float64)
+    for n in range(nt):
+        w1 = uh[n - 1] if n >= 1 else 0.0
+        w2 = uh[n - 2] if n >= 2 else 0.0
+        I += ((uh[n] - 2.0 * w1) + w2) / (float(dt) * float(dt)) * vh[n]
     return I
 
 

@@ -13,7 +13,7 @@ _LIBPATH = os.path.join(_HERE, "csrc", "librtm.so")
 _lib = None
 
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
-           "rtm_set_probes", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
+           "rtm_set_probes", "rtm_probes_dtt_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
            "rtm_export_coeff", "rtm_debug_stamps", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
 
@@ -53,6 +53,7 @@ def load_library():
     lib.rtm_coeffs_host.argtypes = [cfgp] + [vp] * 10
     lib.rtm_set_model.argtypes = [vp] * 8
     lib.rtm_set_probes.argtypes = [vp] * 4
+    lib.rtm_probes_dtt_host.argtypes = [ip, ip, C.c_double, vp, vp]
     lib.rtm_forward_probe.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp]
     lib.rtm_adjoint_image.argtypes = [vp, ip, vp, vp, ip, vp, vp, fp, ip, vp, vp]
     lib.rtm_offset_gather.argtypes = [vp, ip, vp, fp, vp, vp]
@@ -124,6 +125,14 @@ def coeffs_host(cfg: RtmConfig, vp, eps=None, delta=None, theta=None):
     _check(lib.rtm_coeffs_host(C.byref(cfg), _hp(vp), _hp(eps), _hp(delta), _hp(theta), _hp(K2),
                                _hp(outs[0]), _hp(outs[1]), _hp(outs[2]), _hp(outs[3]), _hp(damp)))
     return K2, outs[0], outs[1], outs[2], outs[3], damp
+
+
+def probes_dtt_host(Z, dt):
+    """rtm_probes_dtt_host: Zdd [nt][r] such that probing with Zdd accumulates Z^T u_tt (Eq. 2-3)."""
+    Z = np.ascontiguousarray(Z, np.float32)
+    out = np.empty_like(Z)
+    _check(load_library().rtm_probes_dtt_host(Z.shape[0], Z.shape[1], float(dt), _hp(Z), _hp(out)))
+    return out
 
 
 class Rtm:

@@ -310,6 +310,20 @@ extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const f
     return RTM_OK;
 }
 
+// ---- reading C4: second time difference moved from the wavefield onto the probes (host, fp64) ------------
+extern "C" int rtm_probes_dtt_host(int nt, int r, double dt, const float *h_Z, float *h_Zdd) {
+    if (nt < 1 || r < 1 || !(dt > 0.0) || !h_Z || !h_Zdd || h_Z == h_Zdd) return RTM_EINVAL;
+    const double s = 1.0 / (dt * dt);
+    for (int n = 0; n < nt; n++)
+        for (int k = 0; k < r; k++) {
+            const double z0 = h_Z[(size_t)n * r + k];
+            const double z1 = n + 1 < nt ? (double)h_Z[(size_t)(n + 1) * r + k] : 0.0;
+            const double z2 = n + 2 < nt ? (double)h_Z[(size_t)(n + 2) * r + k] : 0.0;
+            h_Zdd[(size_t)n * r + k] = (float)(((z0 - 2.0 * z1) + z2) * s);
+        }
+    return RTM_OK;
+}
+
 static int launch_pack(rtm_ctx *c, const float *src, float *dst, cudaStream_t st) {
     const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pz;
     pack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, st>>>(c->L, src, dst);

@@ -164,3 +164,34 @@ def test_pdl_off_gives_identical_bits():
     b = run_gpu(p, options={"pdl": 0})
     for k in ("data", "Uz", "Vz", "image"):
         assert np.array_equal(a[k], b[k])
+
+
+@pytest.mark.parametrize("T", [0, 16])
+def test_gradient_imaging_condition_with_dtt_probes(T):
+    """Eq. 2-3 as printed (probe u_tt): Zf = rtm_probes_dtt_host(Z), Za = Z.  The library's Zdd equals the oracle's
+    bit for bit; compressed wavefields and image against the oracle; r = nt identity probes against the exact
+    gradient image from stored histories."""
+    import oracle as orc
+    from paper_2201_06914_b200 import Rtm, probes_dtt_host
+    p = ri.random_acoustic(2, n=(60, 52), nb=8, nt=96, r=6, seed=41, nsrc=1, nrec=9)
+    co = orc.coeffs(p)
+    for Z in (p.Z, ri.identity_probes(p.nt)):
+        r = Z.shape[1]
+        Zdd = probes_dtt_host(Z, p.dt)
+        assert np.array_equal(Zdd, orc.probes_dtt(Z, p.dt))
+        m = Rtm.from_problem(p, r=r, probe_block=T)
+        m.set_model_from_earth(p.vp)
+        m.set_probes(Zdd, Z)
+        data = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+        din = data.cpu().numpy()
+        img, _ = m.adjoint_image(p.rec_xyz, din, p.src_xyz)
+        Uz, Vz = m.export_probes(0).cpu().numpy(), m.export_probes(1).cpu().numpy()
+        img = img.cpu().numpy().ravel()
+        m.close()
+        f = orc.forward(p, co, Z=Zdd, want_hist=True)
+        a = orc.adjoint(p, co, din, Z=Z, want_hist=True)
+        I = orc.image(f["PZ"], a["PZ"], 1.0 / r)
+        assert rel(Uz, f["PZ"]) <= 1e-4 and rel(Vz, a["PZ"]) <= 1e-4 and rel(img, I) <= 1e-4
+        if r == p.nt:
+            Iex = orc.exact_gradient_image(f["hist"], a["hist"], p.dt) * (float(Z[0, 0]) ** 2 / p.nt)
+            assert rel(img, Iex) <= 1e-4

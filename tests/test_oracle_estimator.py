@@ -142,3 +142,41 @@ def test_offset_gather_3d_layout():
     ref = np.zeros(n)
     ref[1:-1] = (U[:, 2:] * V[:, :-2]).sum(0)
     assert np.allclose(G[0].reshape(n), ref, rtol=1e-14, atol=1e-14)
+
+
+# ---- gradient-type imaging condition, Eq. 2-3 as printed: probe u_tt (reading C4) ----------
+def test_dtt_probes_summation_by_parts_exact():
+    """sum_n z[n] (w[n] - 2 w[n-1] + w[n-2]) / dt^2 == sum_n Zdd[n] w[n] (w[-1] = w[-2] = 0, z[nt] = z[nt+1] = 0).
+    Rademacher z and dt = 2^-9 make every Zdd entry an exact fp32 number, so the identity holds to rounding of the
+    fp64 sums; a wrong shift, sign or boundary term in probes_dtt fails it."""
+    rng = np.random.default_rng(5)
+    nt, r, N, dt = 37, 3, 11, 2.0 ** -9
+    Z = rng.choice([-1.0, 1.0], size=(nt, r)).astype(np.float32)
+    w = rng.standard_normal((nt, N))
+    Zdd = orc.probes_dtt(Z, dt).astype(np.float64)
+    wp = np.vstack([np.zeros((2, N)), w])                                  # wp[n + 2] = w[n]
+    dtt = (wp[2:] - 2.0 * wp[1:-1] + wp[:-2]) / dt ** 2                    # [nt][N], available at step n
+    lhs = Z.astype(np.float64).T @ dtt
+    rhs = Zdd.T @ w
+    assert np.abs(lhs - rhs).max() <= 1e-12 * np.abs(lhs).max()
+    # closed form: w[n] = (n + 1)^2, w[-1] = w[-2] = 0: second differences 1, 4 - 2 = 2, then 2 from step 2 on
+    q = ((np.arange(nt) + 1.0) ** 2)[:, None]
+    one = np.ones((nt, 1), np.float32)
+    got = (orc.probes_dtt(one, 1.0).astype(np.float64).T @ q)[0, 0]
+    assert got == 1.0 + 2.0 + 2.0 * (nt - 2)
+
+
+def test_identity_probes_give_exact_gradient_image(tiny):
+    """r = nt, Z = sqrt(nt) I: (1/r) sum_k (Zdd^T u)_k (Z^T v)_k == sum_n u_tt[n] v[n] from stored histories.
+    Zdd is rounded to fp32 like every probe the GPU receives, so the identity holds to fp32 rounding of Zdd."""
+    p, co, f, a, din = tiny
+    Z = ri.identity_probes(p.nt)
+    Zdd = orc.probes_dtt(Z, p.dt)
+    fz = orc.forward(p, co, Z=Zdd)
+    az = orc.adjoint(p, co, din, Z=Z)
+    I = orc.image(fz["PZ"], az["PZ"], 1.0 / p.nt)
+    Iex = orc.exact_gradient_image(f["hist"], a["hist"], p.dt) * (float(Z[0, 0]) ** 2 / p.nt)
+    assert np.abs(I - Iex).max() <= 5e-7 * np.abs(Iex).max()
+    # and it is NOT the zero-lag image: the two conditions differ (sign and spectrum)
+    I0 = orc.exact_image(f["hist"], a["hist"])
+    assert np.abs(Iex / np.abs(Iex).max() - I0 / np.abs(I0).max()).max() > 0.1
