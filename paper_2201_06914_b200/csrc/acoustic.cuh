@@ -23,7 +23,7 @@ namespace rtm {
 // TM = 0: probe fused into every step (or no probing); TM = 4|8|16: time-blocked probing (history ring +
 // fused flush slices of up to TM slots).
 template <int ND, int TM>
-__global__ void __launch_bounds__(256, 4) acoustic_step_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(256, ND == 2 ? 4 : 3) acoustic_step_kernel(const StepArgs a) {
     extern __shared__ __align__(16) float dyn_smem[];
     pdl_launch_dependents();
     const Layout &L = a.L;
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(256, 4) acoustic_step_kernel(const StepArgs a)
         if (ix >= 0 && ix < L.nx && iy >= 0 && iy < L.ny && iz >= 0 && iz < L.nz) {
             const long long o = ((long long)ix * L.ny + iy) * L.upz + iz;
             if (TM > 0) stcs4(a.hist + o, unew);
-            else probe_quad(a.PZ + o, L.Nu, a.Zrow, a.r, unew);
+            else probe_quad<(ND == 2 ? 1 : 2)>(a.PZ + o, L.Nu, a.Zrow, a.r, unew);
         }
     }
 }

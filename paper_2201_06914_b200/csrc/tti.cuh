@@ -23,7 +23,7 @@ constexpr int TTI_GX = TTI_TX + 8, TTI_GZ = TTI_TZ + 8;     // product tile (hal
 constexpr int TTI_SMEM = (2 * TTI_FX * TTI_FZ + 4 * TTI_GX * TTI_GZ) * 4;
 
 template <int TM>
-__global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const StepArgs a) {
     extern __shared__ __align__(16) float smem[];
     float *sA = smem;                          // [FX][FZ]
     float *sB = sA + TTI_FX * TTI_FZ;
@@ -214,7 +214,7 @@ __global__ void __launch_bounds__(256, 4) tti_step_kernel(const StepArgs a) {
             const long long o = (long long)ix * L.upz + iz;
             const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
             if (TM > 0) stcs4(a.hist + o, v);
-            else probe_quad(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+            else probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
         }
     }
 }
