@@ -203,7 +203,7 @@ def kernel_name(p, T):
     if p.physics == 1:
         return "tti_step_kernel<%d>" % (0 if T <= 1 else 16 if T > 8 else 8 if T > 4 else 4)
     if T <= 1:
-        return "acoustic_step_kernel<%d, 0>" % p.ndim
+        return "acoustic_step_kernel<%d>" % p.ndim
     return "acoustic2d_stream_kernel" if p.ndim == 2 else "acoustic3d_stream_kernel"
 
 

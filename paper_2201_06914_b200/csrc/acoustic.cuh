@@ -1,5 +1,6 @@
 // acoustic.cuh -- isotropic acoustic time step (a1) with fused damping, source injection (a3),
-// deferred receiver sampling (a4) and probe accumulation (a5).  2D and 3D.
+// deferred receiver sampling (a4) and the probe accumulated in EVERY step (a5; schedule (A) of DESIGN.md,
+// probe_block <= 1).  2D and 3D.  Time-blocked probing uses acoustic2d_stream.cuh / acoustic3d_stream.cuh.
 //
 //   du_new = K1 du + K2 * sum_axes sum_j w_j (u[+j] - 2u + u[-j])      (increment form of O2:
 //   u_new  = u + du_new                                                 du = u_cur - u_prev)
@@ -20,20 +21,13 @@ namespace rtm {
         s[3] += (P.w - c.w) + (M.w - c.w);              \
     }
 
-// TM = 0: probe fused into every step (or no probing); TM = 4|8|16: time-blocked probing (history ring +
-// fused flush slices of up to TM slots).
-template <int ND, int TM>
+template <int ND>
 __global__ void __launch_bounds__(256, ND == 2 ? 4 : 3) acoustic_step_kernel(const StepArgs a) {
-    extern __shared__ __align__(16) float dyn_smem[];
     pdl_launch_dependents();
     const Layout &L = a.L;
     const int tid = threadIdx.y * 32 + threadIdx.x;
-    if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
-        flush_role<(TM > 0 ? TM : 1)>(a, dyn_smem, tid, 256, blockIdx.x);
-        return;
-    }
     pdl_wait();
-    const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
+    const unsigned lin_block = blockIdx.x;
     sample_points(a, lin_block, 256, tid);
     const unsigned bx = lin_block % a.gx, byz = lin_block / a.gx;
     const unsigned by = byz % a.gy, bz = byz / a.gy;
@@ -97,12 +91,11 @@ __global__ void __launch_bounds__(256, ND == 2 ? 4 : 3) acoustic_step_kernel(con
     const float4 unew = make_float4(un[0], un[1], un[2], un[3]);
     st4(a.n0 + off, unew);
 
-    if (TM > 0 ? (a.hist != nullptr) : (a.PZ != nullptr)) {
+    if (a.PZ != nullptr) {
         const int ix = jx - L.nb, iy = jy - L.nby, iz = jz - L.nb;
         if (ix >= 0 && ix < L.nx && iy >= 0 && iy < L.ny && iz >= 0 && iz < L.nz) {
             const long long o = ((long long)ix * L.ny + iy) * L.upz + iz;
-            if (TM > 0) stcs4(a.hist + o, unew);
-            else probe_quad<(ND == 2 ? 1 : 2)>(a.PZ + o, L.Nu, a.Zrow, a.r, unew);
+            probe_quad<(ND == 2 ? 1 : 2)>(a.PZ + o, L.Nu, a.Zrow, a.r, unew);
         }
     }
 }

@@ -589,14 +589,14 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
         }
     } else if (c->cfg.ndim == 2) {
         switch (tm) {
-            case 0: return launch_ex(c, acoustic_step_kernel<2, 0>, a, nb, block, 0, st);
+            case 0: return launch_ex(c, acoustic_step_kernel<2>, a, nb, block, 0, st);
             case 4: return launch_ex(c, stream2d_fn<4>(c->rx), a, nb, block, smem, st);
             case 8: return launch_ex(c, stream2d_fn<8>(c->rx), a, nb, block, smem, st);
             default: return launch_ex(c, stream2d_fn<16>(c->rx), a, nb, block, smem, st);
         }
     } else {
         switch (tm) {
-            case 0: return launch_ex(c, acoustic_step_kernel<3, 0>, a, nb, block, 0, st);
+            case 0: return launch_ex(c, acoustic_step_kernel<3>, a, nb, block, 0, st);
             case 4: return launch_ex(c, acoustic3d_stream_kernel<4, true>, a, nb, block, smem, st);
             case 8: return launch_ex(c, acoustic3d_stream_kernel<8, true>, a, nb, block, smem, st);
             default: return (c->opt_dbg & 32) ? launch_ex(c, acoustic3d_stream_kernel<16, false>, a, nb, block, smem, st)
