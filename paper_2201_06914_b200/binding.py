@@ -138,7 +138,7 @@ def probes_dtt_host(Z, dt):
 class Rtm:
     """One context = one (model, acquisition size) on one GPU.  Same calls as include/rtm.h."""
 
-    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0", probe_block=0):
+    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0", probe_block=0, guard_bytes=0):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -148,7 +148,14 @@ class Rtm:
         nbytes = workspace_bytes(self.cfg)
         if nbytes == 0:
             raise RTMError(-1, "rtm error -1: invalid config")
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        # Optional guard bands around the caller-owned workspace (tests only): filled with a byte pattern that
+        # check_guards() verifies after a run -- an out-of-bounds WRITE of any kernel next to the workspace shows up.
+        self._guard = int(guard_bytes) // 256 * 256
+        self._alloc = torch.empty(nbytes + 2 * self._guard, dtype=torch.uint8, device=self.device)
+        if self._guard:
+            self._alloc[:self._guard] = 0xAB
+            self._alloc[self._guard + nbytes:] = 0xAB
+        self.workspace = self._alloc[self._guard:self._guard + nbytes]
         h_ = C.c_void_p()
         _check(self.lib.rtm_create(C.byref(self.cfg), self.workspace.data_ptr(), nbytes, C.byref(h_)))
         self.ctx = h_
@@ -160,10 +167,18 @@ class Rtm:
         self._keep = []
 
     @classmethod
-    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None, probe_block=0):
+    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None, probe_block=0, guard_bytes=0):
         mp = max(len(p.src_xyz), len(p.rec_xyz)) if max_pts is None else max_pts
         return cls(p.ndim, p.n, p.h, p.nb, p.physics, p.nt if nt is None else nt, p.dt,
-                   p.r if r is None else r, mp, device=device, probe_block=probe_block)
+                   p.r if r is None else r, mp, device=device, probe_block=probe_block, guard_bytes=guard_bytes)
+
+    def check_guards(self) -> bool:
+        """True if the guard bands around the workspace still hold their pattern (see __init__)."""
+        if not self._guard:
+            return True
+        self.torch.cuda.synchronize(self.device)
+        lo, hi = self._alloc[:self._guard], self._alloc[self._guard + self.workspace.numel():]
+        return bool((lo == 0xAB).all().item()) and bool((hi == 0xAB).all().item())
 
     def close(self):
         if getattr(self, "ctx", None):

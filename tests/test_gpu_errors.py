@@ -92,3 +92,42 @@ def test_no_receivers_and_no_image():
     assert img is None
     torch.cuda.synchronize()
     m.close()
+
+
+@pytest.mark.parametrize("T", [0, 8, 16])
+def test_no_kernel_writes_outside_the_workspace_or_its_outputs(T):
+    """compute-sanitizer is closed on this pool: guard bands around the caller-owned workspace and around every
+    output buffer must keep their pattern after a whole shot (all step kernels, flush roles, image, both gather
+    kernels), on grids with ragged tiles in every direction."""
+    import numpy as np
+    import torch
+    import rtm_inputs as ri
+    from paper_2201_06914_b200 import Rtm
+    cases = [ri.random_acoustic(2, n=(70, 61), nb=8, nt=40, r=6, seed=31, nsrc=2, nrec=5),
+             ri.random_acoustic(3, n=(21, 18, 37), nb=8, nt=36, r=5, seed=32),
+             ri.random_tti(n=(75, 67), nb=12, nt=40, r=9, seed=33)]
+    G = 1 << 16
+
+    def guarded(shape):
+        n = int(np.prod(shape))
+        buf = torch.full((n + 2 * G,), float("nan"), dtype=torch.float32, device="cuda")
+        return buf, buf[G:G + n].view(*shape)
+
+    for p in cases:
+        m = Rtm.from_problem(p, probe_block=T, guard_bytes=1 << 20)
+        m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        m.set_probes(p.Z)
+        bd, data = guarded((p.nt, len(p.rec_xyz)))
+        bi, img = guarded(p.n)
+        offs = np.arange(-4, 5, dtype=np.int32)
+        bg, gat = guarded((len(offs),) + tuple(p.n))
+        bg2, gat2 = guarded((3,) + tuple(p.n))
+        m.forward_probe(p.src_xyz, p.wav, p.rec_xyz, data_out=data)
+        m.adjoint_image(p.rec_xyz, data, p.src_xyz, image=img)
+        m.offset_gather(offs, out=gat)                               # tiled kernel
+        m.offset_gather(np.array([-2, 0, 3], np.int32), out=gat2)    # generic kernel
+        assert m.check_guards()
+        for buf, view in ((bd, data), (bi, img), (bg, gat), (bg2, gat2)):
+            assert torch.isnan(buf[:G]).all() and torch.isnan(buf[-G:]).all()
+            assert torch.isfinite(view).all()
+        m.close()
