@@ -153,6 +153,24 @@ def test_time_blocked_probing_3d_and_tti(T):
     check_all(q, snap_steps=[76], probe_block=T)
 
 
+@pytest.mark.parametrize("T", [5, 16])
+def test_streaming_kernels_multi_tile(T):
+    """Time-blocked schedule on grids that span several tiles / chunks of the streaming kernels with ragged edges:
+    3D: two z tiles (128 + 10), two y tiles, two x chunks of 32 planes; 2D: several row chunks, ragged z quads;
+    off-grid sources and receivers (8 / 4 corners, several entries per injection row)."""
+    p3 = ri.random_acoustic(3, n=(40, 9, 130), nb=4, nt=50, r=8, seed=4, nsrc=2, nrec=9)
+    check_all(p3, snap_steps=[5, 25, 49], offsets=np.arange(-4, 5, dtype=np.int32), probe_block=T)
+    p2 = ri.random_acoustic(2, n=(130, 257), nb=12, nt=120, r=9, seed=3, nsrc=3, nrec=7)
+    check_all(p2, snap_steps=[10, 60, 119], offsets=np.array([-3, 0, 2], np.int32), probe_block=T)
+
+
+def test_c4_and_c2_cropped_time_blocked():
+    p = ri.make_c4(n=(72, 64, 56), nt=200, r=16, nb=16, rec_stride=4)
+    check_all(p, snap_steps=[50, 199], probe_block=16)
+    q = ri.make_c2(n=(240, 176), nt=500, r=64, nb=40)
+    check_all(q, snap_steps=[100, 499], offsets=np.array([-4, 0, 4], np.int32), probe_block=16)
+
+
 def test_c1_cropped_time_blocked():
     p = ri.make_c3(n=(256, 200), nt=600, r=32, nb=80)
     check_all(p, snap_steps=[599], offsets=p.offsets, probe_block=8)
