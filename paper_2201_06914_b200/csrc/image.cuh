@@ -202,7 +202,7 @@ template <int T>
 __global__ void __launch_bounds__(256) probe_flush_kernel(Layout L, const float *__restrict__ hist, int ncur,
                                                           const float *__restrict__ Z0, long long zstep, int zr,
                                                           int r, float *__restrict__ PZ) {
-    __shared__ __align__(16) float sz[T * 256];   // [T][zr], zr <= 256
+    __shared__ __align__(16) float sz[(T <= 16 ? T : 16) * 256];   // [T][zr]; zr <= 256 (T <= 16), zr <= 128 (T = 32)
     for (int i = threadIdx.x; i < T * zr; i += 256) {
         const int j = i / zr, k = i % zr;
         sz[i] = j < ncur ? Z0[j * zstep + k] : 0.0f;

@@ -90,7 +90,9 @@ static bool valid_cfg(const rtm_config *c) {
     if (c->physics != 0 && c->physics != 1) return false;
     if (c->physics == 1 && c->ndim != 2) return false;
     if (c->nt < 1 || c->r < 1 || c->r > 256 || c->max_pts < 1) return false;
-    if (c->probe_block < 0 || c->probe_block > 16) return false;
+    // time blocks of up to 16 steps; the 3D streaming kernel has the registers for 32 history values per thread
+    if (c->probe_block < 0 || c->probe_block > ((c->ndim == 3 && c->physics == 0) ? 32 : 16)) return false;
+    if (c->probe_block > 16 && c->r > 128) return false;   // staging of the 32 Z rows in the final flush kernel
     return true;
 }
 
@@ -548,7 +550,7 @@ static int pick_rx(rtm_ctx *c) {
     return 4;
 }
 
-static int tm_of(int T) { return T <= 0 ? 0 : T <= 4 ? 4 : T <= 8 ? 8 : 16; }
+static int tm_of(int T) { return T <= 0 ? 0 : T <= 4 ? 4 : T <= 8 ? 8 : T <= 16 ? 16 : 32; }
 
 template <typename K>
 static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, dim3 block, size_t smem, cudaStream_t st) {
@@ -599,8 +601,9 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
             case 0: return launch_ex(c, acoustic_step_kernel<3>, a, nb, block, 0, st);
             case 4: return launch_ex(c, acoustic3d_stream_kernel<4, true>, a, nb, block, smem, st);
             case 8: return launch_ex(c, acoustic3d_stream_kernel<8, true>, a, nb, block, smem, st);
-            default: return (c->opt_dbg & 32) ? launch_ex(c, acoustic3d_stream_kernel<16, false>, a, nb, block, smem, st)
-                                             : launch_ex(c, acoustic3d_stream_kernel<16, true>, a, nb, block, smem, st);
+            case 16: return (c->opt_dbg & 32) ? launch_ex(c, acoustic3d_stream_kernel<16, false>, a, nb, block, smem, st)
+                                              : launch_ex(c, acoustic3d_stream_kernel<16, true>, a, nb, block, smem, st);
+            default: return launch_ex(c, acoustic3d_stream_kernel<32, true>, a, nb, block, smem, st);
         }
     }
 }
@@ -611,7 +614,8 @@ static int launch_flush(rtm_ctx *c, const float *hist, int ncur, const float *Z0
     const unsigned nb = (unsigned)((tot + 255) / 256);
     if (c->T <= 4) probe_flush_kernel<4><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
     else if (c->T <= 8) probe_flush_kernel<8><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
-    else probe_flush_kernel<16><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    else if (c->T <= 16) probe_flush_kernel<16><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
+    else probe_flush_kernel<32><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
     c->launches++;
     return RTM_OK;
 }

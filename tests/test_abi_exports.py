@@ -59,7 +59,9 @@ def test_c4_workspace_fits_hbm_where_full_history_does_not():
         w = B.workspace_bytes(B.make_config(probe_block=T, **base))
         assert 2 * 16 * N * 4 + extra <= w <= 2 * 16 * N * 4 + extra + 3.0e9      # + 3 fields, K2, tables
         assert w < 0.15 * hbm and w < full_history / 40
-    assert B.workspace_bytes(B.make_config(probe_block=17, **base)) == 0            # invalid config -> 0
+    assert B.workspace_bytes(B.make_config(probe_block=33, **base)) == 0            # invalid config -> 0
+    base2 = dict(base, ndim=2, n=(512, 256, 0))
+    assert B.workspace_bytes(B.make_config(probe_block=17, **base2)) == 0           # 2D: time blocks of <= 16 steps
 
 
 def test_table1_memory_ratios_golden():

@@ -145,6 +145,13 @@ def test_time_blocked_probing_acoustic2d(T):
     check_all(p, snap_steps=[40, 82], offsets=np.array([-2, 0, 1], np.int32), probe_block=T)
 
 
+def test_time_block_of_32_steps_3d():
+    p = ri.random_acoustic(3, n=(21, 18, 37), nb=8, nt=77, r=5, seed=32)      # two full blocks + a ragged one
+    check_all(p, snap_steps=[76], offsets=np.array([-1, 0, 2], np.int32), probe_block=32)
+    p = ri.random_acoustic(3, n=(40, 9, 130), nb=4, nt=30, r=8, seed=4, nsrc=2, nrec=9)   # nt < T: one ragged block
+    check_all(p, snap_steps=[29], probe_block=27)
+
+
 @pytest.mark.parametrize("T", [4, 8])
 def test_time_blocked_probing_3d_and_tti(T):
     p = ri.random_acoustic(3, n=(21, 18, 37), nb=8, nt=45, r=5, seed=32)
