@@ -228,7 +228,7 @@ def run_ours(args):
 
     p = make_problem(args.workload, args.nt)
     offs = p.offsets
-    T = args.probe_block if args.probe_block >= 0 else (32 if p.ndim == 3 else 16)
+    T = args.probe_block if args.probe_block >= 0 else (32 if p.physics == 0 else 16)
     units = float(p.Np) * p.nt * 2
 
     def barrier():
@@ -320,7 +320,7 @@ def run_ours(args):
     # headline is time-blocked, and vice versa): 1 warm-up + 2 timed shots ----------------------------------
     other = None
     if args.variants:
-        T2 = 0 if T > 1 else (32 if p.ndim == 3 else 16)
+        T2 = 0 if T > 1 else (32 if p.physics == 0 else 16)
         m2 = make_ctx(T2)
         m2.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
         shot2 = shot_on(m2)
@@ -392,7 +392,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c1", choices=["c0", "c1", "c2", "c4"])
     ap.add_argument("--probe-block", type=int, default=-1,
-                    help="T_b of time-blocked probing (default 16, 32 for the 3D workload; 0/1 = probe fused into every step)")
+                    help="T_b of time-blocked probing (default 32 acoustic, 16 TTI; 0/1 = probe fused into every step)")
     ap.add_argument("--variants", type=int, default=1, help="also time the other probe variant (2 shots)")
     ap.add_argument("--pdl", type=int, default=1)
     ap.add_argument("--rx", type=int, default=0)

@@ -45,7 +45,7 @@ typedef struct {
     int r;          /* number of probing vectors, 1..256 (Eq. 1)                    */
     int max_pts;    /* upper bound on nsrc and nrec of any later call (sizes geometry tables)     */
     int probe_block;/* T_b: 0|1 = probe fused into every time step (8 r bytes/point/step of Uz traffic);
-                       2..16 (2..32 for 3D acoustic with r <= 128) = time-blocked probing: each step stores its field into a T_b-slot history
+                       2..16 (2..32 for acoustic physics with r <= 128) = time-blocked probing: each step stores its field into a T_b-slot history
                        ring and every T_b steps one flush applies T_b rows of Z (traffic / T_b).
                        Same sums, same order per (k,x); costs 2 T_b N floats of workspace (the ring is
                        double-buffered: one half is filled while the other is flushed).             */

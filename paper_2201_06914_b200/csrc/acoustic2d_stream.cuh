@@ -27,7 +27,9 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
     const int tid = threadIdx.x;
     if (blockIdx.x < (unsigned)a.fl_blocks) {
         pdl_launch_dependents();
-        flush_role4<TM>(a, dyn_smem, tid, 128, blockIdx.x);
+        // up to 16 history values as float4 per thread; 32 as float2 (register budget), two groups in flight
+        if constexpr (TM <= 16) flush_role4<TM>(a, dyn_smem, tid, 128, blockIdx.x);
+        else flush_role<TM, 2>(a, dyn_smem, tid, 128, blockIdx.x);
         return;
     }
     const unsigned lin_block = blockIdx.x - a.fl_blocks;

@@ -151,7 +151,7 @@ __device__ __forceinline__ void stcs2(float *p, float2 v) { __stcs(reinterpret_c
 
 // Flush role (time-blocked probing): PZ[k][x] += sum_{j<n} Z[n_j][k] hist[j][x] for this block's share of
 // the slice, one float2 of x per thread; T history values stay in registers while r planes stream through.
-template <int TM>
+template <int TM, int DEPTH = 1>
 __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid, int nthreads, int block) {
     const Layout &L = a.L;
     const int zr = a.zr, n = a.fl_n, r = a.r;
@@ -175,31 +175,42 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
 #pragma unroll
         for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs2(a.fl_hist + j * L.Nu + o) : make_float2(0.f, 0.f);
         float *p = a.PZ + o;
-        // software-pipelined over groups of 4 planes: the loads of group g+1 are issued BEFORE the stores
-        // of group g (the compiler cannot hoist them itself: it cannot prove the planes do not alias).  A deeper
-        // pipeline (2 groups in flight) was measured and did not pay inside the 64-register budget of the
-        // 256-thread kernels.
-        float2 nxt[4];
+        // software-pipelined over groups of 4 planes, DEPTH groups in flight: the loads of later groups are issued
+        // BEFORE the stores of the current one (the compiler cannot hoist them itself: it cannot prove the planes do
+        // not alias).  DEPTH 2 did not pay inside the 64-register budget of the 256-thread kernels (DEPTH 1 there);
+        // the 128-thread 2D kernel uses 2 with T = 32.
+        constexpr int G = 4;
+        float2 ring[DEPTH][G];
 #pragma unroll
-        for (int i = 0; i < 4; i++) nxt[i] = (i < r) ? ldcs2(p + (long long)i * L.Nu) : make_float2(0.f, 0.f);
-        for (int k = 0; k < r; k += 4) {   // Z rows are zero-padded to zr (multiple of 8)
-            float2 acc[4];
+        for (int s = 0; s < DEPTH; s++)
 #pragma unroll
-            for (int i = 0; i < 4; i++) acc[i] = nxt[i];
+            for (int i = 0; i < G; i++)
+                ring[s][i] = (s * G + i < r) ? ldcs2(p + (long long)(s * G + i) * L.Nu) : make_float2(0.f, 0.f);
+        for (int kk = 0; kk < r; kk += G * DEPTH) {   // Z rows are zero-padded to zr (multiple of 8)
 #pragma unroll
-            for (int i = 0; i < 4; i++)
-                nxt[i] = (k + 4 + i < r) ? ldcs2(p + (long long)(k + 4 + i) * L.Nu) : make_float2(0.f, 0.f);
+            for (int s = 0; s < DEPTH; s++) {
+                const int k = kk + s * G;
+                if (k >= r) break;
+                float2 acc[G];
 #pragma unroll
-            for (int j = 0; j < TM; j++) {
-                const float4 z = ld4(sz + j * zr + k);
-                acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
-                acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
-                acc[2].x = fmaf(z.z, h[j].x, acc[2].x); acc[2].y = fmaf(z.z, h[j].y, acc[2].y);
-                acc[3].x = fmaf(z.w, h[j].x, acc[3].x); acc[3].y = fmaf(z.w, h[j].y, acc[3].y);
+                for (int i = 0; i < G; i++) acc[i] = ring[s][i];
+#pragma unroll
+                for (int i = 0; i < G; i++) {
+                    const int kn = k + G * DEPTH + i;
+                    ring[s][i] = (kn < r) ? ldcs2(p + (long long)kn * L.Nu) : make_float2(0.f, 0.f);
+                }
+#pragma unroll
+                for (int j = 0; j < TM; j++) {
+                    const float4 z = ld4(sz + j * zr + k);
+                    acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
+                    acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
+                    acc[2].x = fmaf(z.z, h[j].x, acc[2].x); acc[2].y = fmaf(z.z, h[j].y, acc[2].y);
+                    acc[3].x = fmaf(z.w, h[j].x, acc[3].x); acc[3].y = fmaf(z.w, h[j].y, acc[3].y);
+                }
+#pragma unroll
+                for (int i = 0; i < G; i++)
+                    if (k + i < r) stcs2(p + (long long)(k + i) * L.Nu, acc[i]);
             }
-#pragma unroll
-            for (int i = 0; i < 4; i++)
-                if (k + i < r) stcs2(p + (long long)(k + i) * L.Nu, acc[i]);
         }
     }
 }

@@ -90,8 +90,9 @@ static bool valid_cfg(const rtm_config *c) {
     if (c->physics != 0 && c->physics != 1) return false;
     if (c->physics == 1 && c->ndim != 2) return false;
     if (c->nt < 1 || c->r < 1 || c->r > 256 || c->max_pts < 1) return false;
-    // time blocks of up to 16 steps; the 3D streaming kernel has the registers for 32 history values per thread
-    if (c->probe_block < 0 || c->probe_block > ((c->ndim == 3 && c->physics == 0) ? 32 : 16)) return false;
+    // time blocks of up to 16 steps; the acoustic streaming kernels have the registers for 32 history values per
+    // flush-role thread, the TTI kernel (64 registers) has not
+    if (c->probe_block < 0 || c->probe_block > (c->physics == 0 ? 32 : 16)) return false;
     if (c->probe_block > 16 && c->r > 128) return false;   // staging of the 32 Z rows in the final flush kernel
     return true;
 }
@@ -534,11 +535,11 @@ static int pick_rx(rtm_ctx *c) {
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const int tm = tm_of(c->T);
     // flush-role blocks that share every launch: one float4 of the physical grid per thread, 1/T of it per step
-    const long long quads = (long long)c->L.nx * c->L.ny * (c->L.upz / 4);
+    const long long quads = (long long)c->L.nx * c->L.ny * (c->L.upz / (c->T <= 16 ? 4 : 2));
     const long long fblocks = (quads / std::max(1, c->T - 1) + 127) / 128 + 1;
     const int cand[4] = {2, 4, 8, 16};
     for (int i = 0; i < 4; i++) {
-        step_fn f = tm <= 4 ? stream2d_fn<4>(cand[i]) : tm <= 8 ? stream2d_fn<8>(cand[i]) : stream2d_fn<16>(cand[i]);
+        step_fn f = tm <= 4 ? stream2d_fn<4>(cand[i]) : tm <= 8 ? stream2d_fn<8>(cand[i]) : tm <= 16 ? stream2d_fn<16>(cand[i]) : stream2d_fn<32>(cand[i]);
         int per_sm = 0;
         cudaFuncSetAttribute((const void *)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, 128, stream_smem(c, cand[i])) != cudaSuccess) { cudaGetLastError(); continue; }
@@ -594,7 +595,8 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
             case 0: return launch_ex(c, acoustic_step_kernel<2>, a, nb, block, 0, st);
             case 4: return launch_ex(c, stream2d_fn<4>(c->rx), a, nb, block, smem, st);
             case 8: return launch_ex(c, stream2d_fn<8>(c->rx), a, nb, block, smem, st);
-            default: return launch_ex(c, stream2d_fn<16>(c->rx), a, nb, block, smem, st);
+            case 16: return launch_ex(c, stream2d_fn<16>(c->rx), a, nb, block, smem, st);
+            default: return launch_ex(c, stream2d_fn<32>(c->rx), a, nb, block, smem, st);
         }
     } else {
         switch (tm) {
@@ -655,7 +657,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     step_grid(c, &grid, &block, &smem);
     const long long nblocks = (long long)grid.x * grid.y * grid.z;
     const long long bthreads = (long long)block.x * block.y * block.z;
-    const int fl_vec = c->rx ? 4 : 2;   // floats per flush-role thread (flush_role4 in the 2D streaming kernel)
+    const int fl_vec = (c->rx && T <= 16) ? 4 : 2;   // floats per flush-role thread (flush_role4 in the 2D streaming kernel)
     const long long units = (long long)L.nx * L.ny * (L.upz / fl_vec);
     a.gx = grid.x; a.gy = grid.y;
     if (c->rx) a.gx = (unsigned)((L.Pz + 3) / 4);   // streaming kernel: quads per row

@@ -60,8 +60,8 @@ def test_c4_workspace_fits_hbm_where_full_history_does_not():
         assert 2 * 16 * N * 4 + extra <= w <= 2 * 16 * N * 4 + extra + 3.0e9      # + 3 fields, K2, tables
         assert w < 0.15 * hbm and w < full_history / 40
     assert B.workspace_bytes(B.make_config(probe_block=33, **base)) == 0            # invalid config -> 0
-    base2 = dict(base, ndim=2, n=(512, 256, 0))
-    assert B.workspace_bytes(B.make_config(probe_block=17, **base2)) == 0           # 2D: time blocks of <= 16 steps
+    base2 = dict(base, ndim=2, n=(512, 256, 0), physics=1)
+    assert B.workspace_bytes(B.make_config(probe_block=17, **base2)) == 0           # TTI: time blocks of <= 16 steps
 
 
 def test_table1_memory_ratios_golden():

@@ -1,5 +1,5 @@
 """-m gpu tests at BASELINE.json's full grid sizes, in the launch configuration bench.py times (time-blocked
-probing, T = 16).  c1 (2D acoustic, 1751x751, nt = 6000, r = 32, 41 offsets) is compared with the oracle element by
+probing, T = 32 for the acoustic workloads, 16 for TTI).  c1 (2D acoustic, 1751x751, nt = 6000, r = 32, 41 offsets) is compared with the oracle element by
 element over the whole shot; c2 (TTI, 2000x800) over a shortened record; c4 (3D, 512x512x256), which the oracle
 cannot finish in seconds, on sampled outputs the oracle can compute (receiver traces of a cropped-in-time run on a
 sub-volume are covered by test_gpu_parity.py) and on properties that hold at any size: gather[h=0] == image bit for
@@ -25,7 +25,7 @@ def test_c1_full_shot_against_oracle():
     a = orc.adjoint(p, co, din, Z=p.Z)
     img = orc.image(f["PZ"], a["PZ"], 1.0 / p.r)
     gat = orc.offset_gather(p.n, f["PZ"], a["PZ"], p.offsets, 1.0 / p.r)
-    g = run_gpu(p, din=din, offsets=p.offsets, probe_block=16)
+    g = run_gpu(p, din=din, offsets=p.offsets, probe_block=32)
     errs = {"data": rel(g["data"], f["samples"]), "qadj": rel(g["qadj"], a["samples"]), "Uz": rel(g["Uz"], f["PZ"]),
             "Vz": rel(g["Vz"], a["PZ"]), "image": rel(g["image"], img), "gather": rel(g["gather"], gat)}
     print("c1 full", {k: "%.2e" % v for k, v in errs.items()})
@@ -58,7 +58,7 @@ def test_c4_full_grid_properties():
     nt = 24
     p.nt, p.wav, p.Z = nt, np.ascontiguousarray(p.wav[:nt]), np.ascontiguousarray(p.Z[:nt])
     out = {}
-    for T in (16, 0):
+    for T in (32, 0):
         m = Rtm.from_problem(p, probe_block=T)
         m.set_model_from_earth(p.vp)
         m.set_probes(p.Z)
@@ -70,11 +70,11 @@ def test_c4_full_grid_properties():
         m.close()
         del m, data, img, gat
         torch.cuda.empty_cache()
-    d16, i16, g16 = out[16]
+    d16, i16, g16 = out[32]
     d0, i0, g0 = out[0]
     assert np.array_equal(g16[0], i16) and np.array_equal(g0[0], i0)       # gather[h=0] == image
     assert np.abs(i16).max() > 0 and np.abs(d16).max() > 0
-    # the streaming kernel (T = 16) and the plain kernel (T = 0) are different code paths of the same scheme
+    # the streaming kernel (T = 32) and the plain kernel (T = 0) are different code paths of the same scheme
     assert rel(d16, d0) <= TOL_FIELD and rel(i16, i0) <= TOL_IMAGE and rel(g16[1], g0[1]) <= TOL_IMAGE
     # sampled outputs against the oracle: the forward pass of the full grid for the same 24 steps (about half a minute of CPU)
     f = orc.forward(p, orc.coeffs(p))

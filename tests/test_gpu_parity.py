@@ -145,7 +145,10 @@ def test_time_blocked_probing_acoustic2d(T):
     check_all(p, snap_steps=[40, 82], offsets=np.array([-2, 0, 1], np.int32), probe_block=T)
 
 
-def test_time_block_of_32_steps_3d():
+def test_time_block_of_32_steps():
+    p2 = ri.random_acoustic(2, n=(70, 61), nb=8, nt=83, r=6, seed=31, nsrc=2, nrec=5)
+    check_all(p2, snap_steps=[40, 82], offsets=np.array([-2, 0, 1], np.int32), probe_block=32)
+    check_all(p2, snap_steps=[82], probe_block=21)
     p = ri.random_acoustic(3, n=(21, 18, 37), nb=8, nt=77, r=5, seed=32)      # two full blocks + a ragged one
     check_all(p, snap_steps=[76], offsets=np.array([-1, 0, 2], np.int32), probe_block=32)
     p = ri.random_acoustic(3, n=(40, 9, 130), nb=4, nt=30, r=8, seed=4, nsrc=2, nrec=9)   # nt < T: one ragged block
