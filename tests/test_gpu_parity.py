@@ -240,3 +240,36 @@ def test_gradient_imaging_condition_with_dtt_probes(T):
         if r == p.nt:
             Iex = orc.exact_gradient_image(f["hist"], a["hist"], p.dt) * (float(Z[0, 0]) ** 2 / p.nt)
             assert rel(img, Iex) <= 1e-4
+
+
+def test_multi_shot_stacking_in_place():
+    """survey loop with in-place image accumulation (rtm_adjoint_image accumulate = 1,
+    PAPER.md:L73/L85 "stack"): three shots through one context against the sum of the oracle's images."""
+    import types
+    import torch
+    import oracle as orc
+    from paper_2201_06914_b200 import Rtm
+    from paper_2201_06914_b200.survey import migrate_shots
+    p = ri.random_acoustic(2, n=(60, 52), nb=8, nt=90, r=6, seed=51, nsrc=1, nrec=9)
+    co = orc.coeffs(p)
+    rng = np.random.default_rng(3)
+    shots, Isum = [], 0.0
+    for s in range(3):
+        src = np.array([[rng.uniform(0.1, 0.9) * (p.n[0] - 1) * p.h, rng.uniform(0.0, 0.3) * (p.n[1] - 1) * p.h]], np.float32)
+        f = orc.propagate(p, co, False, src, p.wav, p.rec_xyz, Z=p.Z)
+        din = f["samples"].astype(np.float32)
+        a = orc.propagate(p, co, True, p.rec_xyz, din, src, Z=p.Z)
+        Isum = Isum + orc.image(f["PZ"], a["PZ"], 1.0 / p.r)
+        shots.append(types.SimpleNamespace(src_xyz=src, wav=p.wav, rec_xyz=p.rec_xyz, data_in=din))
+    m = Rtm.from_problem(p, probe_block=32)
+    m.set_model_from_earth(p.vp)
+    m.set_probes(p.Z)
+    image = torch.zeros(p.n, dtype=torch.float32, device="cuda")
+    assert migrate_shots(m, shots, image) == 3
+    assert rel(image.cpu().numpy(), Isum) <= 1e-4
+    # accumulate = 0 overwrites
+    img1, _ = m.adjoint_image(shots[2].rec_xyz, shots[2].data_in, shots[2].src_xyz, image=image, accumulate=False)
+    last = orc.image(orc.propagate(p, co, False, shots[2].src_xyz, p.wav, p.rec_xyz, Z=p.Z)["PZ"],
+                     orc.propagate(p, co, True, p.rec_xyz, shots[2].data_in, shots[2].src_xyz, Z=p.Z)["PZ"], 1.0 / p.r)
+    assert rel(img1.cpu().numpy(), last) <= 1e-4
+    m.close()
