@@ -77,7 +77,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -87,6 +87,11 @@ class ClockSampler:
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append(line.strip())
+
+    def mark(self):
+        """Forget the samples taken so far (the sampler is started before the warm-up so that it is already
+        running when the timed region begins)."""
+        self.rows = []
 
     def stop(self):
         if self.proc is None:
@@ -286,11 +291,13 @@ def run_ours(args):
         return shot
 
     shot = shot_on(m)
-    for _ in range(args.warmup):
-        shot()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for _ in range(args.warmup):
+        shot()
+    torch.cuda.synchronize()
+    sampler.mark()                       # only samples taken during the timed region count
     l0 = m.launch_count()
     ms = timed(shot, args.steps)
     launches = m.launch_count() - l0
