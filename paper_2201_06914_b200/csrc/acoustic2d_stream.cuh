@@ -33,6 +33,7 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
         return;
     }
     const unsigned lin_block = blockIdx.x - a.fl_blocks;
+    DBG_STAMP(a, 0);   // timing experiments (dbg & 16): block start / before the wait / after it / end
     // flattened task index: (row chunk, z-quad) pairs are dealt to consecutive threads, so no lane idles
     // on a ragged Pz; a.gx = number of z-quads per row
     const unsigned task = lin_block * 128u + tid;
@@ -109,7 +110,9 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
     }
     const bool zdamp = (dzv[0] != 0.f) | (dzv[1] != 0.f) | (dzv[2] != 0.f) | (dzv[3] != 0.f);
 
+    DBG_STAMP(a, 1);
     pdl_wait();   // from here on the previous step's fields are complete and visible
+    DBG_STAMP(a, 2);
     // Dependents are released only now: a block of step n+1 can therefore only start once step n-1 is complete,
     // which is what lets the flush role of step n+1 skip its own wait (see flush_role4) and overlap with step n.
     pdl_launch_dependents();
@@ -231,6 +234,7 @@ __global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_con
         if (zphys && ix >= 0 && ix < L.nx) stcs4(a.hist + (long long)ix * L.upz + iz, un);
     }
     }   // active
+    DBG_STAMP(a, 6);
 }
 
 }  // namespace rtm

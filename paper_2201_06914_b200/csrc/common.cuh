@@ -149,6 +149,17 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ float2 ldcs2(const float *p) { return __ldcs(reinterpret_cast<const float2 *>(p)); }
 __device__ __forceinline__ void stcs2(float *p, float2 v) { __stcs(reinterpret_cast<float2 *>(p), v); }
 
+__device__ __forceinline__ unsigned long long gtimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define DBG_STAMP(a, slot)                                                                  \
+    do {                                                                                    \
+        if (((a).dbg & 16) && threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x < 1024)    \
+            (a).dbg_ts[blockIdx.x * 8 + (slot)] = gtimer();                                 \
+    } while (0)
+
 // Flush role (time-blocked probing): PZ[k][x] += sum_{j<n} Z[n_j][k] hist[j][x] for this block's share of
 // the slice, one float2 of x per thread; T history values stay in registers while r planes stream through.
 template <int TM, int DEPTH = 1>
@@ -164,7 +175,9 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
     // the slices on slots >= 1 of the time block) and the stencil blocks release their dependents only after their
     // own wait, so every launch <= n-2 is complete when a block of launch n runs: no wait needed, and the role
     // overlaps with the previous step instead of starting behind it.
+    DBG_STAMP(a, 0);
     if (!a.fl_nowait) pdl_wait();
+    DBG_STAMP(a, 2);
     const int np = L.upz / 2;
     for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
         const long long row = t / np;
@@ -213,6 +226,7 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
             }
         }
     }
+    DBG_STAMP(a, 6);
 }
 
 // Same role with one float4 of x per thread (fewer, fatter threads: used by the 2D streaming kernel, whose
@@ -227,7 +241,9 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
         sz[i] = j < n ? a.fl_Z0[j * a.fl_zstep + k] : 0.0f;
     }
     __syncthreads();
+    DBG_STAMP(a, 0);
     if (!a.fl_nowait) pdl_wait();   // see flush_role
+    DBG_STAMP(a, 2);
     const int nq = L.upz / 4;
     for (long long t = a.fl_q0 + (long long)block * nthreads + tid; t < a.fl_q1; t += (long long)a.fl_blocks * nthreads) {
         const long long row = t / nq;
@@ -275,18 +291,8 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
             }
         }
     }
+    DBG_STAMP(a, 6);
 }
-
-__device__ __forceinline__ unsigned long long gtimer() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define DBG_STAMP(a, slot)                                                                  \
-    do {                                                                                    \
-        if (((a).dbg & 16) && threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x < 1024)    \
-            (a).dbg_ts[blockIdx.x * 8 + (slot)] = gtimer();                                 \
-    } while (0)
 
 __device__ __forceinline__ float k1_of(float s) { return s == 0.0f ? 1.0f : (1.0f - s) / (1.0f + s); }
 // Deferred receiver sampling: the first ceil(nsmp/nthreads) blocks (linear order) take one point
