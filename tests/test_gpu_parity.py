@@ -116,13 +116,14 @@ def test_run_to_run_repeatable():
         assert np.array_equal(a[k], b[k])
 
 
-def test_shot_host_matches_device_calls():
+@pytest.mark.parametrize("T", [0, 32])
+def test_shot_host_matches_device_calls(T):
     import torch
     from paper_2201_06914_b200 import Rtm
     p = ri.random_acoustic(2, n=(50, 44), nb=8, nt=60, r=8, seed=13)
     offs = np.array([-2, 0, 3], np.int32)
-    g = run_gpu(p, offsets=offs)
-    m = Rtm.from_problem(p)
+    g = run_gpu(p, offsets=offs, probe_block=T)
+    m = Rtm.from_problem(p, probe_block=T)
     m.set_model_from_earth(p.vp)
     m.set_probes(p.Z)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
