@@ -305,6 +305,11 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     value = world * units * args.steps / (ms * 1e-3)
 
+    # ---- the offset-gather kernel alone, for its own roofline line ----------------------------
+    gather_ms = None
+    if offs is not None:
+        gather_ms = timed(lambda: m.offset_gather(offs, out=gather), 10) / 10
+
     # ---- end to end: host buffers through rtm_shot_host ------------------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_wav, h_din = pin(p.wav), din.cpu().pin_memory()
@@ -381,6 +386,11 @@ def run_ours(args):
                        "ms_per_step": ms_e / ke},
                "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
                "pass_ms": {"forward_steps": fwd_ms, "adjoint_steps": adj_ms}}
+        if gather_ms is not None:
+            gb = 8.0 * p.r * p.N + 4.0 * len(offs) * p.N          # Uz, Vz read once + the volume written once
+            out["gather"] = {"kernel": "gather_tiled_kernel", "nh": int(len(offs)), "ms": gather_ms,
+                             "min_bytes": gb, "achieved": gb / (gather_ms * 1e-3) / 1e9, "unit": "GB/s",
+                             "frac": gb / (gather_ms * 1e-3) / 1e9 / peak}
         if other is not None:
             T2, ms2, f2, a2 = other
             out["variant"] = {"probe": "per-step fused" if T2 <= 1 else "time-blocked, T=%d" % T2,

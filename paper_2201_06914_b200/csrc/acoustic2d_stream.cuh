@@ -20,8 +20,10 @@
 
 namespace rtm {
 
+// 4 blocks of 128 threads per SM = 128 registers: without the bound the compiler takes 136 - 142 and the launch loses a
+// quarter of its resident blocks (measured: 12.2 us per step instead of 10.1 at c1).
 template <int TM, int RX>
-__global__ void __launch_bounds__(128) acoustic2d_stream_kernel(const __grid_constant__ StepArgs a) {
+__global__ void __launch_bounds__(128, 4) acoustic2d_stream_kernel(const __grid_constant__ StepArgs a) {
     extern __shared__ __align__(16) float dyn_smem[];
     const Layout &L = a.L;
     const int tid = threadIdx.x;
