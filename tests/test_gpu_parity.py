@@ -274,3 +274,13 @@ def test_multi_shot_stacking_in_place():
                      orc.propagate(p, co, True, p.rec_xyz, shots[2].data_in, shots[2].src_xyz, Z=p.Z)["PZ"], 1.0 / p.r)
     assert rel(img1.cpu().numpy(), last) <= 1e-4
     m.close()
+
+
+def test_rademacher_probes():
+    """PAPER.md:L33 names Rademacher probing vectors (entries +-1): Z is an input of the library (reading C2), so
+    the same kernels must reproduce the oracle with them; with +-1 probes the per-step products are exact."""
+    p = ri.random_acoustic(2, n=(64, 50), nb=8, nt=70, r=8, seed=61, nsrc=1, nrec=7)
+    p.Z = ri.rademacher_probes(p.nt, p.r, seed=7)
+    assert set(np.unique(p.Z)) == {-1.0, 1.0}
+    for T in (0, 32):
+        check_all(p, offsets=np.arange(-4, 5, dtype=np.int32), probe_block=T)
