@@ -199,6 +199,21 @@ def offset_gather(n, Uz, Vz, offsets, scale):
     return G
 
 
+def offset_gather_xy(n, Uz, Vz, offsets_xy, scale):
+    """Eq. 4 with vector offsets h = (hx, hy) on a 3D grid n = (nx, ny, nz): [nh][N] (reading C28)."""
+    lib = _load()
+    r, N = Uz.shape
+    nx, ny, nz = (int(v) for v in n)
+    assert N == nx * ny * nz
+    Uz = np.ascontiguousarray(Uz, np.float64)
+    Vz = np.ascontiguousarray(Vz, np.float64)
+    offs = np.ascontiguousarray(offsets_xy, np.int32).reshape(-1, 2)
+    G = np.zeros((len(offs), N), np.float64)
+    lib.orc_offset_gather_xy(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_int(r), _fp(Uz), _fp(Vz),
+                             C.c_int(len(offs)), _fp(offs), C.c_double(scale), _fp(G))
+    return G
+
+
 def tti_H(p, co, which, f):
     """Test hook: H_perp (which=0) / H_par (which=1) applied to a padded-grid function [Np]."""
     lib = _load()

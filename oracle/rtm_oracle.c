@@ -21,7 +21,7 @@
  *
  * Pins (tests/test_oracle_*.py): Z = sqrt(nt) I  =>  image == exact image; Uz == history^T Z via
  * numpy matmul; estimator mean/variance closed form (Avron-Toledo); gather[h=0] == image, brute
- * force gather; dot test <Fq,d> = <q,F^T d>; analytic 2D/3D Green's functions incl. 2nd-order
+ * force gather (scalar and vector offsets; spike pair at midpoint / half-offset); dot test <Fq,d> = <q,F^T d>; analytic 2D/3D Green's functions incl. 2nd-order
  * convergence in dt; TTI: H symmetric negative semi-definite, eps=delta=theta=0 => p == r ==
  * acoustic, theta -> theta+pi invariance; coefficient closed forms.
  * PARITY UNPINNED (free choices no external fact fixes): the damping profile shape and strength,
@@ -472,6 +472,29 @@ void orc_offset_gather(int nx, long nrest /* ny*nz */, int r, const double *Uz, 
                         s += Uz[(long)k * N + (long)a * nrest + q] * Vz[(long)k * N + (long)b * nrest + q];
                 G[(long)ih * N + (long)ix * nrest + q] = scale * s;
             }
+    }
+}
+
+/* Eq. 4 with a VECTOR horizontal offset h = (hx, hy) in grid points (
+ * PAPER.md:L81 "generalize to 3D"; reading C26): 3D grids [nx][ny][nz],
+ * G[ih][x] = scale * sum_k Uz[k][x + hx e_x + hy e_y] Vz[k][x - hx e_x - hy e_y];
+ * zero when either shifted point leaves [0,nx) x [0,ny).  offs = [nh][2] = (hx, hy) pairs.         */
+void orc_offset_gather_xy(int nx, int ny, int nz, int r, const double *Uz, const double *Vz, int nh,
+                          const int *offs, double scale, double *G) {
+    long N = (long)nx * ny * nz;
+    for (int ih = 0; ih < nh; ih++) {
+        int hx = offs[2 * ih], hy = offs[2 * ih + 1];
+        for (int ix = 0; ix < nx; ix++)
+            for (int iy = 0; iy < ny; iy++)
+                for (int iz = 0; iz < nz; iz++) {
+                    int ax = ix + hx, ay = iy + hy, bx = ix - hx, by = iy - hy;
+                    double s = 0.0;
+                    if (ax >= 0 && ax < nx && ay >= 0 && ay < ny && bx >= 0 && bx < nx && by >= 0 && by < ny)
+                        for (int k = 0; k < r; k++)
+                            s += Uz[(long)k * N + ((long)ax * ny + ay) * nz + iz] *
+                                 Vz[(long)k * N + ((long)bx * ny + by) * nz + iz];
+                    G[(long)ih * N + ((long)ix * ny + iy) * nz + iz] = scale * s;
+                }
     }
 }
 

@@ -144,6 +144,86 @@ def test_offset_gather_3d_layout():
     assert np.allclose(G[0].reshape(n), ref, rtol=1e-14, atol=1e-14)
 
 
+# ---- vector-offset volumes, Eq. 4 with h = (hx, hy) (reading C28) --------------------------
+def _shifted(A, hx, hy):
+    """A[:, ix + hx, iy + hy, :] with zeros outside the grid, by padding + slicing (no index arithmetic shared
+    with the oracle)."""
+    r, nx, ny, nz = A.shape
+    P = max(abs(hx), abs(hy), 1)
+    B = np.zeros((r, nx + 2 * P, ny + 2 * P, nz))
+    B[:, P:P + nx, P:P + ny] = A
+    return B[:, P + hx:P + hx + nx, P + hy:P + hy + ny]
+
+
+def test_offset_gather_xy_point_pair_sign_and_axes():
+    """One spike in Uz at a, one in Vz at b: Eq. 4 is non-zero only at the midpoint x = (a + b)/2 with
+    h = (a - b)/2.  A swapped sign of h, swapped U/V roles or swapped x/y axes moves or kills the spike."""
+    n = (9, 7, 3)
+    a, b = (6, 5, 1), (2, 1, 1)                       # midpoint (4, 3, 1), h = (+2, +2)
+    U = np.zeros((1,) + n)
+    V = np.zeros((1,) + n)
+    U[0][a] = 3.0
+    V[0][b] = 5.0
+    offs = np.array([[2, 2], [-2, -2], [2, -2], [-2, 2], [2, 0], [0, 2], [0, 0]], np.int32)
+    G = orc.offset_gather_xy(n, U.reshape(1, -1), V.reshape(1, -1), offs, 1.0).reshape(len(offs), *n)
+    assert G[0][4, 3, 1] == 15.0 and np.count_nonzero(G[0]) == 1
+    assert not G[1:].any()
+    # asymmetric pair: only hx differs from zero
+    a, b = (7, 3, 2), (1, 3, 2)                       # midpoint (4, 3, 2), h = (+3, 0)
+    U[:] = 0
+    V[:] = 0
+    U[0][a] = 2.0
+    V[0][b] = 7.0
+    offs = np.array([[3, 0], [0, 3], [-3, 0]], np.int32)
+    G = orc.offset_gather_xy(n, U.reshape(1, -1), V.reshape(1, -1), offs, 0.5).reshape(3, *n)
+    assert G[0][4, 3, 2] == 7.0 and np.count_nonzero(G[0]) == 1 and not G[1:].any()
+
+
+def test_offset_gather_xy_against_padded_slices_and_identities():
+    rng = np.random.default_rng(21)
+    n = (7, 6, 4)
+    r = 3
+    N = int(np.prod(n))
+    Uz = rng.standard_normal((r, N))
+    Vz = rng.standard_normal((r, N))
+    offs = np.array([[0, 0], [1, 0], [0, 1], [-2, 3], [3, -2], [6, 0], [0, -5], [7, 0], [0, 6], [-1, -1]], np.int32)
+    G = orc.offset_gather_xy(n, Uz, Vz, offs, 1.0 / r)
+    U4, V4 = Uz.reshape(r, *n), Vz.reshape(r, *n)
+    for ih, (hx, hy) in enumerate(offs):
+        ref = (_shifted(U4, hx, hy) * _shifted(V4, -hx, -hy)).sum(0) / r
+        assert np.allclose(G[ih].reshape(n), ref, rtol=1e-13, atol=1e-14), (hx, hy)
+    assert np.array_equal(G[0], orc.image(Uz, Vz, 1.0 / r))                 # PAPER.md:L52: h = 0 is the image
+    assert not G[7].any() and not G[8].any()                                # |h| >= n: no valid pair left
+    assert G[5].any() is not None
+    # hy = 0 reduces to the scalar-offset volumes of the north_star
+    hx_only = np.array([-3, -1, 0, 2], np.int32)
+    Gx = orc.offset_gather(n, Uz, Vz, hx_only, 1.0 / r)
+    Gxy = orc.offset_gather_xy(n, Uz, Vz, np.stack([hx_only, 0 * hx_only], 1), 1.0 / r)
+    assert np.array_equal(Gx, Gxy)
+    # exchanging the roles of the two wavefields mirrors the offset
+    Gm = orc.offset_gather_xy(n, Vz, Uz, -offs, 1.0 / r)
+    assert np.allclose(G, Gm, rtol=1e-14, atol=1e-15)
+
+
+def test_offset_gather_xy_equals_exact_extended_image_for_orthonormal_probes():
+    """(1/r) Z Z^T = I (Z = sqrt(nt) I, reading C1)  =>  Eq. 4's estimate IS the exact extended image
+    sum_t u[t][x + h] v[t][x - h], here for vector h."""
+    rng = np.random.default_rng(22)
+    n = (5, 4, 3)
+    nt = 6
+    N = int(np.prod(n))
+    uh = rng.standard_normal((nt, N))
+    vh = rng.standard_normal((nt, N))
+    Z = np.sqrt(nt) * np.eye(nt)
+    Uz, Vz = Z.T @ uh, Z.T @ vh
+    offs = np.array([[1, -1], [0, 2], [-2, 1]], np.int32)
+    G = orc.offset_gather_xy(n, Uz, Vz, offs, 1.0 / nt)
+    u4, v4 = uh.reshape(nt, *n), vh.reshape(nt, *n)
+    for ih, (hx, hy) in enumerate(offs):
+        ref = (_shifted(u4, hx, hy) * _shifted(v4, -hx, -hy)).sum(0)
+        assert np.allclose(G[ih].reshape(n), ref, rtol=1e-12, atol=1e-13)
+
+
 # ---- gradient-type imaging condition, Eq. 2-3 as printed: probe u_tt (reading C4; SURVEY 8(f) item 1) ----------
 def test_dtt_probes_summation_by_parts_exact():
     """sum_n z[n] (w[n] - 2 w[n-1] + w[n-2]) / dt^2 == sum_n Zdd[n] w[n] (w[-1] = w[-2] = 0, z[nt] = z[nt+1] = 0).
