@@ -117,6 +117,16 @@ int rtm_adjoint_image(rtm_ctx *ctx, int nrec, const float *h_rec_xyz, const floa
 int rtm_offset_gather(rtm_ctx *ctx, int nh, const int *h_offsets, float scale, float *d_gather,
                       void *cuda_stream);
 
+/* Eq. 4 with VECTOR horizontal offsets on 3D grids ("h is a vector of horizontal offsets",
+ * L81 "generalize to 3D", reading C28):
+ *   gather[ih][x] = scale * sum_k Uz[k][x + hx e_x + hy e_y] Vz[k][x - hx e_x - hy e_y],
+ *   (hx, hy) = h_offsets_xy[2 ih], h_offsets_xy[2 ih + 1] in grid points (host, [nh][2]); zero where either shifted
+ *   point leaves [0,nx) x [0,ny).  (hx, 0) equals rtm_offset_gather bit for bit, (0, 0) the image.
+ *   d_gather [nh][N] device, caller-owned.  Runs of >= 8 consecutive hx at one hy are served by the register-tiled
+ *   kernel.  Errors: RTM_EINVAL (ndim != 3, nh < 1 or > 4096, |hx| >= nx, |hy| >= ny), RTM_ESTATE (no Uz/Vz yet).  */
+int rtm_offset_gather_xy(rtm_ctx *ctx, int nh, const int *h_offsets_xy, float scale, float *d_gather,
+                         void *cuda_stream);
+
 /* One whole shot from HOST buffers (the end-to-end call): uploads wav and data_in, runs
  * rtm_forward_probe, rtm_adjoint_image and (nh > 0) rtm_offset_gather, downloads data_out, image
  * and gather.  Host buffers should be pinned for true asynchrony.  d_staging: caller-owned device

@@ -14,6 +14,7 @@ _lib = None
 
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
            "rtm_set_probes", "rtm_probes_dtt_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
+           "rtm_offset_gather_xy",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
            "rtm_export_coeff", "rtm_debug_stamps", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
 
@@ -57,6 +58,7 @@ def load_library():
     lib.rtm_forward_probe.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp]
     lib.rtm_adjoint_image.argtypes = [vp, ip, vp, vp, ip, vp, vp, fp, ip, vp, vp]
     lib.rtm_offset_gather.argtypes = [vp, ip, vp, fp, vp, vp]
+    lib.rtm_offset_gather_xy.argtypes = [vp, ip, vp, fp, vp, vp]
     lib.rtm_shot_staging_bytes.restype = C.c_size_t
     lib.rtm_shot_staging_bytes.argtypes = [cfgp, ip, ip, ip]
     lib.rtm_shot_host.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp, fp, vp, ip, vp, vp, vp, C.c_size_t, vp]
@@ -267,6 +269,16 @@ class Rtm:
             out = t.empty((len(offs),) + self.n, dtype=t.float32, device=self.device)
         sc = 1.0 / self.r if scale is None else float(scale)
         _check(self.lib.rtm_offset_gather(self.ctx, len(offs), _hp(offs), sc, self._ptr(out), self._stream()))
+        return out
+
+    def offset_gather_xy(self, offsets_xy, scale=None, out=None):
+        """rtm_offset_gather_xy: offsets_xy [nh][2] = (hx, hy) grid points, 3D grids only."""
+        t = self.torch
+        offs = np.ascontiguousarray(offsets_xy, np.int32).reshape(-1, 2)
+        if out is None:
+            out = t.empty((len(offs),) + self.n, dtype=t.float32, device=self.device)
+        sc = 1.0 / self.r if scale is None else float(scale)
+        _check(self.lib.rtm_offset_gather_xy(self.ctx, len(offs), _hp(offs), sc, self._ptr(out), self._stream()))
         return out
 
     def shot_host(self, src_xyz, h_wav, rec_xyz, h_data_in, h_data_out=None, h_image=None, offsets=None,

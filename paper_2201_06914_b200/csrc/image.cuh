@@ -66,6 +66,45 @@ __global__ void __launch_bounds__(256) gather_kernel(Layout L, const float *__re
     }
 }
 
+// a8 with vector offsets h = (hx, hy) on 3D grids (Eq. 4; reading C28):
+//   G[ih][x] = scale * sum_k Uz[k][x + hx e_x + hy e_y] Vz[k][x - hx e_x - hy e_y], zero where a shifted point leaves
+// [0,nx) x [0,ny).  trip = [nl][3] = (ih, hx, hy): the offsets the register-tiled kernel did not take.
+__global__ void __launch_bounds__(256) gather_xy_kernel(Layout L, const float *__restrict__ U, const float *__restrict__ V,
+                                                        int r, int nl, const int *__restrict__ trip, float scale,
+                                                        float *__restrict__ G) {
+    const int nq = L.upz / 4;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long rows = (long long)L.nx * L.ny;
+    if (t >= rows * nq) return;
+    const long long row = t / nq;
+    const int iz = (int)(t % nq) * 4;
+    if (iz >= L.nz) return;
+    const int ix = (int)(row / L.ny), iy = (int)(row % L.ny);
+    const long long xs = (long long)L.ny * L.upz;
+    const long long o = row * L.upz + iz;
+    const long long N = rows * L.nz;
+    for (int i = 0; i < nl; i++) {
+        const int ih = trip[3 * i], hx = trip[3 * i + 1], hy = trip[3 * i + 2];
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ix + hx >= 0 && ix + hx < L.nx && ix - hx >= 0 && ix - hx < L.nx && iy + hy >= 0 && iy + hy < L.ny &&
+            iy - hy >= 0 && iy - hy < L.ny) {
+            const long long sh = hx * xs + (long long)hy * L.upz;
+            const float *pu = U + o + sh, *pv = V + o - sh;
+#pragma unroll 4
+            for (int k = 0; k < r; k++) {
+                const float4 u = ld4(pu + k * L.Nu), v = ld4(pv + k * L.Nu);
+                acc.x = fmaf(u.x, v.x, acc.x);
+                acc.y = fmaf(u.y, v.y, acc.y);
+                acc.z = fmaf(u.z, v.z, acc.z);
+                acc.w = fmaf(u.w, v.w, acc.w);
+            }
+        }
+        const float res[4] = {acc.x, acc.y, acc.z, acc.w};
+        float *out = G + (long long)ih * N + row * L.nz + iz;
+        for (int q = 0; q < 4 && iz + q < L.nz; q++) out[q] = scale * res[q];
+    }
+}
+
 // a8, register-tiled fast path for a run of consecutive offsets h0, h0+1, ..., h0+nh-1 (nh <= GT_HP).
 //
 // The generic kernel above reads 2 x LDG.128 per 4 FMA and is bound by L1/L2 throughput (c3: 1.39 ms for a 552 MB
@@ -81,7 +120,7 @@ constexpr int GT_SMEM = 2 * 2 * GT_ROWS * 32 * 4;
 
 __global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, const float *__restrict__ U,
                                                                    const float *__restrict__ V, int r, int nh, int h0,
-                                                                   float scale, float *__restrict__ G) {
+                                                                   int hy, float scale, float *__restrict__ G) {
     extern __shared__ __align__(16) float gsm[];   // [2 buffers][U | V][GT_ROWS][32]
     const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
     const int xg = grp % (GT_X / 8), hg = grp / (GT_X / 8);
@@ -89,6 +128,12 @@ __global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, cons
     const long long l0 = (long long)blockIdx.x * 32;          // first float of the fast axes
     const int x0 = blockIdx.y * GT_X;
     const int xu0 = x0 + h0, xv0 = x0 - (h0 + GT_HP - 1);     // first x row of the U / V tile
+    // vector offsets (hx, hy) on 3D grids (reading C28): upz % 32 == 0, so the block's 32 floats lie in one y row
+    // iy0 and a shift by hy along y is a shift by hy * upz floats, valid for the whole block or for none of it
+    const int iy0 = (int)(l0 / L.upz);
+    const bool yok = iy0 + hy >= 0 && iy0 + hy < L.ny && iy0 - hy >= 0 && iy0 - hy < L.ny;
+    const long long lu = l0 + (long long)(yok ? hy : 0) * L.upz, lv = l0 - (long long)(yok ? hy : 0) * L.upz;
+    const bool active = hg * 8 < nh;                           // offset groups beyond nh only help with the staging
 
     auto request = [&](int k, int buf) {
         float *dst = gsm + buf * (2 * GT_ROWS * 32);
@@ -97,8 +142,8 @@ __global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, cons
             const int row = c >> 3, q = c & 7;
             const bool isV = row >= GT_ROWS;
             const int x = isV ? xv0 + (row - GT_ROWS) : xu0 + row;
-            const bool ok = x >= 0 && x < L.nx;
-            const float *src = (isV ? V : U) + (long long)k * L.Nu + (long long)(ok ? x : 0) * R + l0 + q * 4;
+            const bool ok = yok && x >= 0 && x < L.nx;
+            const float *src = (isV ? V : U) + (long long)k * L.Nu + (long long)(ok ? x : 0) * R + (isV ? lv : lu) + q * 4;
             cp_async16(dst + row * 32 + q * 4, src, ok);
         }
         cp_async_commit();
@@ -115,6 +160,7 @@ __global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, cons
         cp_async_wait<0>();
         __syncthreads();            // probe k has landed for everybody; nobody still reads the other buffer
         if (k + 1 < r) request(k + 1, (k + 1) & 1);
+        if (!active) continue;
         const float *us = gsm + (k & 1) * (2 * GT_ROWS * 32) + (8 * (xg + hg)) * 32 + lane;
         const float *vs = gsm + (k & 1) * (2 * GT_ROWS * 32) + (GT_ROWS + 8 * xg - 8 * hg + GT_HP - 8) * 32 + lane;
         float u[15], v[15];

@@ -150,7 +150,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t o_rs = take((size_t)(nrows + 1) * 4);
     size_t o_en = take((size_t)c->max_pts * nc * sizeof(InjEntry));
     size_t o_si = take((size_t)c->max_pts * nc * 4), o_sw = take((size_t)c->max_pts * nc * 4);
-    size_t o_of = take(4096 * 4);
+    size_t o_of = take(3 * 4096 * 4);
     size_t o_dbg = take(1024 * 8 * 8);
     if (ctx) {
         char *b = ctx->ws;
@@ -236,7 +236,7 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
         CU(cudaMallocHost(&h.smp_w, (size_t)cfg->max_pts * nc * 4));
         CU(cudaEventCreateWithFlags(&h.done, cudaEventDisableTiming));
     }
-    CU(cudaMallocHost(&c->h_offs, 4096 * 4));
+    CU(cudaMallocHost(&c->h_offs, 3 * 4096 * 4));
     CU(cudaEventCreateWithFlags(&c->offs_done, cudaEventDisableTiming));
     *out = c;
     return RTM_OK;
@@ -796,12 +796,55 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
     for (int i = 1; i < nh && run; i++) run = h_offsets[i] == h_offsets[i - 1] + 1;
     if (run) {
         const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
-        gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, h_offsets[0], scale, d_gather);
+        gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, h_offsets[0], 0, scale, d_gather);
     } else {
         const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
         gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, c->offs, scale, d_gather);
     }
     c->launches++;
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
+extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy, float scale, float *d_gather, void *stream) {
+    if (!c || nh < 1 || nh > 4096 || !h_offsets_xy || !d_gather || c->cfg.ndim != 3) return RTM_EINVAL;
+    if (!c->have_U || !c->have_V) return RTM_ESTATE;
+    for (int i = 0; i < nh; i++)
+        if (std::abs(h_offsets_xy[2 * i]) >= c->cfg.n[0] || std::abs(h_offsets_xy[2 * i + 1]) >= c->cfg.n[1]) return RTM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Layout &L = c->L;
+    const long long N = (long long)L.nx * L.ny * L.nz;
+    if (c->offs_pending) { CU(cudaEventSynchronize(c->offs_done)); c->offs_pending = false; }
+    // runs of consecutive hx at one hy (8..GT_HP long) take the register-tiled kernel, the rest the generic one
+    int nl = 0;
+    for (int i = 0; i < nh;) {
+        int j = i + 1;
+        while (j < nh && j - i < GT_HP && h_offsets_xy[2 * j + 1] == h_offsets_xy[2 * i + 1] &&
+               h_offsets_xy[2 * j] == h_offsets_xy[2 * (j - 1)] + 1)
+            j++;
+        if (j - i >= 8) {
+            const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
+            gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->cfg.r, j - i, h_offsets_xy[2 * i],
+                                                                   h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
+            c->launches++;
+        } else {
+            for (int m = i; m < j; m++) {
+                c->h_offs[3 * nl] = m;
+                c->h_offs[3 * nl + 1] = h_offsets_xy[2 * m];
+                c->h_offs[3 * nl + 2] = h_offsets_xy[2 * m + 1];
+                nl++;
+            }
+        }
+        i = j;
+    }
+    if (nl) {
+        CU(cudaMemcpyAsync(c->offs, c->h_offs, (size_t)nl * 12, cudaMemcpyHostToDevice, st));
+        CU(cudaEventRecord(c->offs_done, st));
+        c->offs_pending = true;
+        const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
+        gather_xy_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nl, c->offs, scale, d_gather);
+        c->launches++;
+    }
     CU(cudaGetLastError());
     return RTM_OK;
 }

@@ -18,7 +18,7 @@ def snap_rel(gs, rs):
     return max(np.linalg.norm(gs[i] - rs[i]) for i in range(len(rs))) / den
 
 
-def run_gpu(p, snap_steps=(), din=None, offsets=None, want_qadj=True, probe_block=0, options=None):
+def run_gpu(p, snap_steps=(), din=None, offsets=None, want_qadj=True, probe_block=0, options=None, offsets_xy=None):
     import torch
     from paper_2201_06914_b200 import Rtm
     m = Rtm.from_problem(p, probe_block=probe_block)
@@ -45,6 +45,8 @@ def run_gpu(p, snap_steps=(), din=None, offsets=None, want_qadj=True, probe_bloc
     out["Vz"] = m.export_probes(1).cpu().numpy()
     if offsets is not None:
         out["gather"] = m.offset_gather(offsets).cpu().numpy().reshape(len(offsets), -1)
+    if offsets_xy is not None:
+        out["gather_xy"] = m.offset_gather_xy(offsets_xy).cpu().numpy().reshape(len(offsets_xy), -1)
     out["launches"] = m.launch_count()
     torch.cuda.synchronize()
     m.close()

@@ -45,6 +45,9 @@ def test_state_and_argument_errors():
     with pytest.raises(RTMError) as e:          # |h| >= nx
         m.offset_gather(np.array([p.n[0]], np.int32))
     assert e.value.code == -1
+    with pytest.raises(RTMError) as e:          # vector offsets are for 3D grids
+        m.offset_gather_xy(np.array([[0, 0]], np.int32))
+    assert e.value.code == -1
     many = np.tile(p.rec_xyz, (4, 1))           # more points than max_pts
     with pytest.raises(RTMError) as e:
         m.forward_probe(p.src_xyz, p.wav, many)

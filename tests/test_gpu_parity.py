@@ -85,6 +85,45 @@ def test_gather_tiled_path(nd, n, nh):
     assert np.array_equal(g2["gather"], g["gather"][::2])
 
 
+@pytest.mark.parametrize("n", [(21, 19, 37), (45, 13, 70)])
+def test_gather_xy_vector_offsets(n):
+    """Eq. 4 with vector offsets (hx, hy) on 3D grids (reading C28) against orc_offset_gather_xy:
+    rows of 11 consecutive hx at one hy take the register-tiled kernel (ragged x tiles, y rows that fall off the
+    grid), scattered pairs and offsets as large as the grid the generic one."""
+    import oracle as orc
+    p = ri.random_acoustic(3, n=n, nb=4, nt=120, r=5, seed=41, nsrc=1, nrec=6)
+    box = [(hx, hy) for hy in range(-3, 4) for hx in range(-5, 6)]
+    extra = [(0, 0), (n[0] - 1, 0), (0, n[1] - 1), (-2, 5), (3, -3), (n[0] // 2, -(n[1] // 2)), (1, 0), (2, 0)]
+    offs = np.array(box + extra, np.int32)
+    hx_line = np.arange(-5, 6, dtype=np.int32)
+    g, o, e = check_all(p, offsets=hx_line)
+    gx = run_gpu(p, offsets_xy=offs)
+    assert np.array_equal(gx["Uz"], g["Uz"]) and np.array_equal(gx["Vz"], g["Vz"])
+    G = gx["gather_xy"]
+    ref = orc.offset_gather_xy(p.n, o["Uz"], o["Vz"], offs, 1.0 / p.r)
+    assert np.abs(ref).max() > 0
+    assert rel(G, ref) <= 1e-4, rel(G, ref)
+    # the gather kernels alone, on the GPU's own compressed wavefields: fp32 dot products of r terms
+    ref2 = orc.offset_gather_xy(p.n, gx["Uz"], gx["Vz"], offs, 1.0 / p.r)
+    assert rel(G, ref2) <= 2e-6, rel(G, ref2)
+    for i in range(len(offs)):                   # per offset, incl. exact zeros where the shift leaves the grid
+        assert np.array_equal(G[i] == 0, ref2[i] == 0) or rel(G[i], ref2[i]) <= 1e-5, offs[i]
+        assert np.linalg.norm(G[i] - ref2[i]) <= 1e-5 * np.linalg.norm(ref2[len(box)]), offs[i]
+    # (hx, 0) == rtm_offset_gather and (0, 0) == the image, bit for bit (PAPER.md:L52)
+    row0 = [i for i, (hx, hy) in enumerate(box) if hy == 0]
+    assert np.array_equal(G[row0], g["gather"])
+    assert np.array_equal(G[len(box)], g["image"])
+    # generic kernel (runs broken up by taking every other pair) == tiled kernel
+    g2 = run_gpu(p, offsets_xy=offs[: len(box)][::2])
+    assert np.array_equal(g2["gather_xy"], G[: len(box)][::2])
+    # exact zeros wherever x + h or x - h leaves [0,nx) x [0,ny) (reading C28), for h and -h alike
+    ix, iy = np.meshgrid(np.arange(n[0]), np.arange(n[1]), indexing="ij")
+    for i, (hx, hy) in enumerate(offs):
+        inside = ((ix + hx >= 0) & (ix + hx < n[0]) & (ix - hx >= 0) & (ix - hx < n[0]) &
+                  (iy + hy >= 0) & (iy + hy < n[1]) & (iy - hy >= 0) & (iy - hy < n[1]))
+        assert not G[i].reshape(n)[~inside].any(), (hx, hy)
+
+
 def test_gather_h0_equals_image_bitwise():
     p = ri.random_acoustic(2, n=(50, 45), nb=8, nt=60, r=6, seed=9)
     g = run_gpu(p, offsets=np.array([0], np.int32))
