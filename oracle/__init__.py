@@ -97,8 +97,9 @@ def coeffs(p, vp=None) -> Coeffs:
 
 
 def propagate(p, co: Coeffs, adjoint: bool, inj_xyz, inj_val, smp_xyz=None, Z=None, want_hist=False,
-              snap_steps=(), nt=None, want_samples=True):
-    """O2/O3/O5/O6.  Returns dict(samples [nt][nsmp], PZ [r][N], hist [nt][N], snaps [ns][nf][Np])."""
+              snap_steps=(), nt=None, want_samples=True, fields=1):
+    """O2/O3/O5/O6.  Returns dict(samples [nt][nsmp], PZ [r][N], hist [nt][N], snaps [ns][nf][Np]).
+    fields=2 (TTI, reading C29): p and r probed apart, PZ [2r][N] (p planes, then r planes), hist [nt][2][N]."""
     lib = _load()
     nt = int(p.nt if nt is None else nt)
     r = 0 if Z is None else int(Z.shape[1])
@@ -115,11 +116,13 @@ def propagate(p, co: Coeffs, adjoint: bool, inj_xyz, inj_val, smp_xyz=None, Z=No
     nf = 2 if p.physics == 1 else 1
     out = np.zeros((nt, nsmp), np.float64) if (want_samples and nsmp > 0) else None
     Zc = _f32(Z)
-    PZ = np.zeros((r, N), np.float64) if r > 0 else None
-    hist = np.zeros((nt, N), np.float64) if want_hist else None
+    assert fields in (1, 2)
+    PZ = np.zeros((fields * r, N), np.float64) if r > 0 else None
+    hist = np.zeros((nt, N) if fields == 1 else (nt, 2, N), np.float64) if want_hist else None
     ss = np.asarray(list(snap_steps), np.int32)
     snaps = np.zeros((len(ss), nf, Np), np.float64) if len(ss) else None
-    rc = lib.orc_propagate(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
+    fn = lib.orc_propagate if fields == 1 else lib.orc_propagate_pr
+    rc = fn(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
                            _fp(co.delh), _fp(co.cosT), _fp(co.sinT), C.c_int(ninj), _fp(inj_xyz), _fp(inj_val),
                            C.c_int(nsmp), _fp(smp_xyz), _fp(out), _fp(Zc), _fp(PZ), _fp(hist),
                            C.c_int(len(ss)), _fp(ss), _fp(snaps))

@@ -23,7 +23,8 @@
  * numpy matmul; estimator mean/variance closed form (Avron-Toledo); gather[h=0] == image, brute
  * force gather (scalar and vector offsets; spike pair at midpoint / half-offset); dot test <Fq,d> = <q,F^T d>; analytic 2D/3D Green's functions incl. 2nd-order
  * convergence in dt; TTI: H symmetric negative semi-definite, eps=delta=theta=0 => p == r ==
- * acoustic, theta -> theta+pi invariance; coefficient closed forms.
+ * acoustic, theta -> theta+pi invariance; coefficient closed forms; two-field TTI probing (C29): central
+ * differences of the misfit in K2 against sum_n (D p w_p + D r w_r) / (K2 h^2) from the histories.
  * PARITY UNPINNED (free choices no external fact fixes): the damping profile shape and strength,
  * the wavelet delay, and imaging the single TTI field (p+r)/2.
  *
@@ -300,16 +301,17 @@ int orc_tti_H(const orc_cfg *c, const float *cosT, const float *sinT, int which,
  * snaps: [nsnap][nf][Np] (nf = 1 acoustic, 2 TTI), the field(s) right after step snap_steps[i]
  * (including that step's injection).
  * Returns 0, or -2 if a position is outside the physical grid.                                   */
-int orc_propagate(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
+static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
                   const float *epsh, const float *delh, const float *cosT, const float *sinT,
                   int ninj, const float *inj_xyz, const float *inj_val /*[nt][ninj]*/,
                   int nsmp, const float *smp_xyz, double *smp_out /*[nt][nsmp] or NULL*/,
-                  const float *Z /*[nt][r] or NULL*/, double *PZ /*[r][N] or NULL*/,
-                  double *hist /*[nt][N] or NULL*/, int nsnap, const int *snap_steps,
-                  double *snaps) {
+                  const float *Z /*[nt][r] or NULL*/, double *PZ /*[np][r][N] or NULL*/,
+                  double *hist /*[nt][np][N] or NULL*/, int nsnap, const int *snap_steps,
+                  double *snaps, int np /* probed fields: 1, or 2 = p and r apart (TTI) */) {
     geom g; make_geom(c, &g);
     const int d = c->ndim, tti = (c->physics == 1);
     if (tti && d != 2) return -1;
+    if (np != 1 && !(np == 2 && tti)) return -1;
     const int nf = tti ? 2 : 1;
     const int nc = 1 << d;
 
@@ -413,11 +415,14 @@ int orc_propagate(const orc_cfg *c, int adjoint, const float *K2, const float *d
                     for (int iz = 0; iz < g.n[2]; iz++) {
                         long i = eidx(&g, ix + layer_of(&g, 0), iy + layer_of(&g, 1), iz + layer_of(&g, 2));
                         long x = ((long)ix * g.n[1] + iy) * g.n[2] + iz;
-                        double u = tti ? 0.5 * (pn[i] + rn[i]) : pn[i];
-                        if (hist) hist[(long)n * g.N + x] = u;
-                        if (PZ && Z)
-                            for (int k = 0; k < c->r; k++)
-                                PZ[(long)k * g.N + x] += (double)Z[(long)n * c->r + k] * u;
+                        for (int f = 0; f < np; f++) {
+                            /* one probed field 1/2 (p + r) (reading C10), or p and r apart (reading C29) */
+                            double u = np == 2 ? (f ? rn[i] : pn[i]) : (tti ? 0.5 * (pn[i] + rn[i]) : pn[i]);
+                            if (hist) hist[((long)n * np + f) * g.N + x] = u;
+                            if (PZ && Z)
+                                for (int k = 0; k < c->r; k++)
+                                    PZ[((long)f * c->r + k) * g.N + x] += (double)Z[(long)n * c->r + k] * u;
+                        }
                     }
         }
         for (int q = 0; q < nsnap; q++)
@@ -437,6 +442,28 @@ int orc_propagate(const orc_cfg *c, int adjoint, const float *K2, const float *d
     free(A); free(B); free(t1); free(t2); free(ma); free(mb);
     free(iE); free(iW); free(sE); free(sW);
     return 0;
+}
+
+int orc_propagate(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
+                  const float *epsh, const float *delh, const float *cosT, const float *sinT,
+                  int ninj, const float *inj_xyz, const float *inj_val, int nsmp, const float *smp_xyz,
+                  double *smp_out, const float *Z, double *PZ /*[r][N]*/, double *hist /*[nt][N]*/, int nsnap,
+                  const int *snap_steps, double *snaps) {
+    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
+                     Z, PZ, hist, nsnap, snap_steps, snaps, 1);
+}
+
+/* Four compressed arrays for the TTI gradient (Eq. 2-3 applied to the coupled (p, r) system of
+ * PAPER.md:L77, reading C29): the same pass, but p and r are probed apart,
+ * PZ [2][r][N] = (Pz, Rz) forward / (Wpz, Wrz) adjoint, hist [nt][2][N].  Eq. 3 over the 2r planes,
+ * (1/r) sum_k (Pz_k Wpz_k + Rz_k Wrz_k), then estimates sum_t (p w_p + r w_r).                            */
+int orc_propagate_pr(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
+                     const float *epsh, const float *delh, const float *cosT, const float *sinT,
+                     int ninj, const float *inj_xyz, const float *inj_val, int nsmp, const float *smp_xyz,
+                     double *smp_out, const float *Z, double *PZ /*[2][r][N]*/, double *hist /*[nt][2][N]*/,
+                     int nsnap, const int *snap_steps, double *snaps) {
+    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
+                     Z, PZ, hist, nsnap, snap_steps, snaps, 2);
 }
 
 /* ==== O4. Images ============================================================================== */

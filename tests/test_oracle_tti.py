@@ -87,3 +87,93 @@ def test_delta_is_clamped_to_epsilon():
     co = orc.coeffs(p)
     assert np.allclose(co.delh, np.sqrt(1.1), rtol=1e-7)
     assert np.allclose(co.epsh, 1.1, rtol=1e-7)
+
+
+# ---- four compressed arrays for the TTI gradient (reading C29) -------------------------------
+def _second_difference(H):
+    """D[n] = H[n] - 2 H[n-1] + H[n-2] with zero fields before step 0; H [nt][...]."""
+    Hp = np.concatenate([np.zeros((2,) + H.shape[1:]), H])
+    return (Hp[2:] - 2.0 * Hp[1:-1]) + Hp[:-2]
+
+
+def test_two_field_gradient_is_the_derivative_of_the_misfit():
+    """What fixes the four-array condition is calculus, not the oracle: for J = 1/2 |F(K2) q - d_obs|^2 and
+    K2 -> K2 (1 + eta) on the physical grid, dJ/d eta(x) = sum_n (D p[n] w_p[n] + D r[n] w_r[n])(x) / (K2(x) h^2),
+    D the undivided second time difference of the stored forward fields and (w_p, w_r) the adjoint fields of the
+    residual.  Central differences of J (the forward pass only) against that sum from the two-field histories: a
+    dropped r term, a swapped field, a wrong time shift or scale all fail.  The one-field image of 1/2 (p + r)
+    (reading C10) is not this gradient and misses by far more than the tolerance."""
+    p = ri.random_tti(n=(34, 30), nb=8, nt=90, r=4, seed=5)
+    co = orc.coeffs(p)
+    rng = np.random.default_rng(3)
+    d0 = orc.forward(p, co)["samples"]
+    dobs = 0.7 * d0 + 0.01 * np.abs(d0).max() * rng.standard_normal(d0.shape)
+
+    def J(K2):
+        d = orc.forward(p, orc.Coeffs(K2, co.damp, co.epsh, co.delh, co.cosT, co.sinT))["samples"]
+        return 0.5 * ((d - dobs) ** 2).sum()
+
+    f = orc.forward(p, co, want_hist=True, fields=2)
+    assert np.array_equal(f["samples"], d0)                       # probing does not touch the propagation
+    a = orc.adjoint(p, co, f["samples"] - dobs, want_hist=True, fields=2)
+    S = (_second_difference(f["hist"]) * a["hist"]).sum(axis=(0, 1))
+    P = (p.n[0] + 2 * p.nb, p.n[1] + 2 * p.nb)
+    K2 = np.asarray(co.K2, np.float64).reshape(P)
+    K2phys = K2[p.nb:-p.nb, p.nb:-p.nb].ravel()
+    g = S / (K2phys * float(np.float32(p.h)) ** 2)
+    eta = rng.standard_normal(p.N)
+    errs = []
+    for t in (1e-2, 3e-3):
+        def pert(sgn):
+            K = K2.copy()
+            K[p.nb:-p.nb, p.nb:-p.nb] *= 1.0 + sgn * t * eta.reshape(p.n)
+            return K.ravel().astype(np.float32)
+        fd = (J(pert(+1)) - J(pert(-1))) / (2 * t)
+        errs.append(abs(fd / (g @ eta) - 1.0))
+    assert errs[1] <= 2e-3, errs
+    assert errs[1] < 0.2 * errs[0], errs                          # O(t^2): it converges to the sum, not near it
+    f1 = orc.forward(p, co, want_hist=True)
+    a1 = orc.adjoint(p, co, f["samples"] - dobs, want_hist=True)
+    S1 = (_second_difference(f1["hist"]) * a1["hist"]).sum(axis=0)
+    g1 = 2.0 * S1 / (K2phys * float(np.float32(p.h)) ** 2)
+    assert abs((g1 @ eta) / (g @ eta) - 1.0) > 0.2
+
+
+def test_two_field_probes_are_history_times_Z_and_split_the_one_field_probe():
+    p = ri.random_tti(n=(30, 26), nb=8, nt=50, r=6, seed=8)
+    co = orc.coeffs(p)
+    f2 = orc.forward(p, co, Z=p.Z, want_hist=True, fields=2)
+    f1 = orc.forward(p, co, Z=p.Z, want_hist=True)
+    Z = p.Z.astype(np.float64)
+    for fld in range(2):                                          # plane block fld == Z^T history of field fld
+        ref = Z.T @ f2["hist"][:, fld, :]
+        assert np.abs(f2["PZ"][fld * p.r:(fld + 1) * p.r] - ref).max() <= 1e-12 * np.abs(ref).max()
+    assert np.abs(f2["hist"][:, 0] - f2["hist"][:, 1]).max() > 0  # anisotropic: p != r
+    assert np.abs(0.5 * (f2["hist"][:, 0] + f2["hist"][:, 1]) - f1["hist"]).max() <= 1e-15 * np.abs(f1["hist"]).max()
+    half = 0.5 * (f2["PZ"][:p.r] + f2["PZ"][p.r:])
+    assert np.abs(half - f1["PZ"]).max() <= 1e-12 * np.abs(f1["PZ"]).max()
+
+
+def test_two_field_identity_probes_give_the_exact_sum_and_the_isotropic_limit():
+    """r = nt, Z = sqrt(nt) I: Eq. 3 over the 2r planes == sum_n (p w_p + r w_r) from the stored histories.
+    eps = delta = 0: p == r and w_p == w_r, so the four-array image is twice the one-field image."""
+    p = ri.random_tti(n=(28, 24), nb=8, nt=40, r=40, seed=9)
+    co = orc.coeffs(p)
+    Z = ri.identity_probes(p.nt)
+    f = orc.forward(p, co, Z=Z, want_hist=True, fields=2)
+    a = orc.adjoint(p, co, f["samples"], Z=Z, want_hist=True, fields=2)
+    I = orc.image(f["PZ"], a["PZ"], 1.0 / p.nt)
+    Iex = (f["hist"] * a["hist"]).sum(axis=(0, 1)) * (float(Z[0, 0]) ** 2 / p.nt)
+    assert np.abs(I - Iex).max() <= 1e-12 * np.abs(Iex).max()
+    p.eps[:] = 0
+    p.delta[:] = 0
+    p.theta[:] = 0
+    p.Z = ri.gaussian_probes(p.nt, 5, 1)
+    p.r = 5
+    co = orc.coeffs(p)
+    f2 = orc.forward(p, co, Z=p.Z, fields=2)
+    a2 = orc.adjoint(p, co, f2["samples"], Z=p.Z, fields=2)
+    f1 = orc.forward(p, co, Z=p.Z)
+    a1 = orc.adjoint(p, co, f2["samples"], Z=p.Z)
+    I2, I1 = orc.image(f2["PZ"], a2["PZ"], 0.2), orc.image(f1["PZ"], a1["PZ"], 0.2)
+    assert np.abs(I1).max() > 0 and np.abs(I2 - 2.0 * I1).max() <= 1e-12 * np.abs(I1).max()
