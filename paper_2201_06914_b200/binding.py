@@ -28,7 +28,7 @@ class RTMError(RuntimeError):
 class RtmConfig(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("h", C.c_float), ("nb", C.c_int),
                 ("physics", C.c_int), ("nt", C.c_int), ("dt", C.c_double), ("r", C.c_int),
-                ("max_pts", C.c_int), ("probe_block", C.c_int)]
+                ("max_pts", C.c_int), ("probe_block", C.c_int), ("probe_fields", C.c_int)]
 
 
 def lib_path() -> str:
@@ -87,7 +87,7 @@ def _check(rc):
         raise RTMError(rc, "rtm error %d: %s" % (rc, msg))
 
 
-def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block=0) -> RtmConfig:
+def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block=0, probe_fields=0) -> RtmConfig:
     c = RtmConfig()
     c.ndim = int(ndim)
     for i, v in enumerate(n):
@@ -100,6 +100,7 @@ def make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block=0) -> R
     c.r = int(r)
     c.max_pts = int(max_pts)
     c.probe_block = int(probe_block)
+    c.probe_fields = int(probe_fields)
     return c
 
 
@@ -140,12 +141,14 @@ def probes_dtt_host(Z, dt):
 class Rtm:
     """One context = one (model, acquisition size) on one GPU.  Same calls as include/rtm.h."""
 
-    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0", probe_block=0, guard_bytes=0):
+    def __init__(self, ndim, n, h, nb, physics, nt, dt, r, max_pts, device="cuda:0", probe_block=0, guard_bytes=0,
+                 probe_fields=0):
         import torch
         self.torch = torch
         self.lib = load_library()
-        self.cfg = make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block)
+        self.cfg = make_config(ndim, n, h, nb, physics, nt, dt, r, max_pts, probe_block, probe_fields)
         self.probe_block = int(probe_block)
+        self.probe_planes = (2 if int(probe_fields) == 2 else 1) * int(r)
         self.device = torch.device(device)
         nbytes = workspace_bytes(self.cfg)
         if nbytes == 0:
@@ -169,10 +172,12 @@ class Rtm:
         self._keep = []
 
     @classmethod
-    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None, probe_block=0, guard_bytes=0):
+    def from_problem(cls, p, device="cuda:0", nt=None, r=None, max_pts=None, probe_block=0, guard_bytes=0,
+                     probe_fields=0):
         mp = max(len(p.src_xyz), len(p.rec_xyz)) if max_pts is None else max_pts
         return cls(p.ndim, p.n, p.h, p.nb, p.physics, p.nt if nt is None else nt, p.dt,
-                   p.r if r is None else r, mp, device=device, probe_block=probe_block, guard_bytes=guard_bytes)
+                   p.r if r is None else r, mp, device=device, probe_block=probe_block, guard_bytes=guard_bytes,
+                   probe_fields=probe_fields)
 
     def check_guards(self) -> bool:
         """True if the guard bands around the workspace still hold their pattern (see __init__)."""
@@ -302,7 +307,7 @@ class Rtm:
 
     def export_probes(self, which):
         t = self.torch
-        out = t.empty((self.r, self.N), dtype=t.float32, device=self.device)
+        out = t.empty((self.probe_planes, self.N), dtype=t.float32, device=self.device)
         _check(self.lib.rtm_export_probes(self.ctx, int(which), self._ptr(out), self._stream()))
         return out
 

@@ -50,6 +50,7 @@ struct StepArgs {
     float *PZ;
     const float *Zrow;
     int r;
+    int two;                // TTI, probe_fields = 2 (reading C29): p -> planes [0, r), r -> planes [r, 2r) of PZ
     // time-blocked probing: instead of PZ, store the probed field into this history slot (physical grid,
     // probe-plane layout); probe_flush_kernel applies T rows of Z at once
     float *hist;

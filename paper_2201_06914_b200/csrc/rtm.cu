@@ -55,6 +55,7 @@ struct rtm_ctx {
     float *k1x, *k1y, *k1z;
     float *Uz, *Vz, *Zf, *Za, *hist;
     int zr, T, rx;
+    int rp;   // probe planes per compressed array: r, or 2 r when p and r are probed apart (probe_fields = 2)
     int *row_start;
     InjEntry *ent;
     int *smp_idx;
@@ -94,6 +95,9 @@ static bool valid_cfg(const rtm_config *c) {
     // flush-role thread, the TTI kernel (64 registers) has not
     if (c->probe_block < 0 || c->probe_block > (c->physics == 0 ? 32 : 16)) return false;
     if (c->probe_block > 16 && c->r > 128) return false;   // staging of the 32 Z rows in the final flush kernel
+    // four compressed arrays for the TTI gradient (reading C29): TTI with the probe fused into every step only
+    if (c->probe_fields != 0 && c->probe_fields != 1 && c->probe_fields != 2) return false;
+    if (c->probe_fields == 2 && (c->physics != 1 || c->probe_block > 1)) return false;
     return true;
 }
 
@@ -138,7 +142,8 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     if (nf == 2) { o_e = take(fb); o_d = take(fb); o_c = take(fb); o_s = take(fb); }
     size_t o_dx = take((size_t)(L.Px + 32) * 4), o_dy = take((size_t)(L.Py + 8) * 4), o_dz = take((size_t)(L.Pz + 8) * 4);
     size_t o_kx = take((size_t)(L.Px + 32) * 4), o_ky = take((size_t)(L.Py + 8) * 4), o_kz = take((size_t)(L.Pz + 8) * 4);
-    size_t pb = (size_t)c->r * (size_t)L.Nu * 4;
+    const int rp = c->probe_fields == 2 ? 2 * c->r : c->r;
+    size_t pb = (size_t)rp * (size_t)L.Nu * 4;
     size_t o_U = take(pb), o_V = take(pb);
     const int T = c->probe_block > 1 ? c->probe_block : 0;
     size_t o_H = take(2 * (size_t)T * (size_t)L.Nu * 4);   // double-buffered history ring
@@ -177,6 +182,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->Zf = (float *)(b + o_Zf);
         ctx->Za = (float *)(b + o_Za);
         ctx->zr = zr;
+        ctx->rp = rp;
         ctx->row_start = (int *)(b + o_rs);
         ctx->ent = (InjEntry *)(b + o_en);
         ctx->smp_idx = (int *)(b + o_si);
@@ -585,7 +591,8 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
     const int tm = tm_of(c->T);
     if (c->cfg.physics == 1) {
         switch (tm) {
-            case 0: return launch_ex(c, tti_step_kernel<0>, a, nb, block, smem, st);
+            case 0: return a.two ? launch_ex(c, tti_step_kernel<0, true>, a, nb, block, smem, st)
+                                 : launch_ex(c, tti_step_kernel<0>, a, nb, block, smem, st);
             case 4: return launch_ex(c, tti_step_kernel<4>, a, nb, block, smem, st);
             case 8: return launch_ex(c, tti_step_kernel<8>, a, nb, block, smem, st);
             default: return launch_ex(c, tti_step_kernel<16>, a, nb, block, smem, st);
@@ -628,7 +635,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     const Layout &L = c->L;
     const int nt = cfg.nt, d = cfg.ndim, T = c->T;
     CU(cudaMemsetAsync(c->fields_base, 0, c->fields_bytes, st));
-    CU(cudaMemsetAsync(PZ, 0, (size_t)cfg.r * (size_t)L.Nu * 4, st));
+    CU(cudaMemsetAsync(PZ, 0, (size_t)c->rp * (size_t)L.Nu * 4, st));
 
     StepArgs a;
     memset(&a, 0, sizeof a);
@@ -639,6 +646,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     a.adjoint = adjoint;
     a.PZ = PZ;
     a.r = cfg.r;
+    a.two = cfg.probe_fields == 2;
     a.row_start = c->row_start;
     a.ent = c->ent;
     double inj_scale = adjoint ? (double)cfg.h * (double)cfg.h : std::pow((double)cfg.h, 2.0 - d);
@@ -755,7 +763,7 @@ extern "C" int rtm_forward_probe(rtm_ctx *c, int nsrc, const float *h_src_xyz, c
 static int launch_image(rtm_ctx *c, float scale, int accumulate, float *d_image, cudaStream_t st) {
     const Layout &L = c->L;
     const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
-    image_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, scale, accumulate, d_image);
+    image_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->rp, scale, accumulate, d_image);
     c->launches++;
     CU(cudaGetLastError());
     return RTM_OK;
@@ -796,10 +804,10 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
     for (int i = 1; i < nh && run; i++) run = h_offsets[i] == h_offsets[i - 1] + 1;
     if (run) {
         const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
-        gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, h_offsets[0], 0, scale, d_gather);
+        gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], 0, scale, d_gather);
     } else {
         const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
-        gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nh, c->offs, scale, d_gather);
+        gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->rp, nh, c->offs, scale, d_gather);
     }
     c->launches++;
     CU(cudaGetLastError());
@@ -824,7 +832,7 @@ extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy,
             j++;
         if (j - i >= 8) {
             const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
-            gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->cfg.r, j - i, h_offsets_xy[2 * i],
+            gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
                                                                    h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
             c->launches++;
         } else {
@@ -842,7 +850,7 @@ extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy,
         CU(cudaEventRecord(c->offs_done, st));
         c->offs_pending = true;
         const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
-        gather_xy_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->cfg.r, nl, c->offs, scale, d_gather);
+        gather_xy_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->rp, nl, c->offs, scale, d_gather);
         c->launches++;
     }
     CU(cudaGetLastError());
@@ -900,8 +908,8 @@ extern "C" int rtm_export_probes(rtm_ctx *c, int which, float *d_out, void *stre
     if (!c || !d_out || (which != 0 && which != 1)) return RTM_EINVAL;
     if (which == 0 ? !c->have_U : !c->have_V) return RTM_ESTATE;
     const Layout &L = c->L;
-    const long long tot = (long long)L.nx * L.ny * L.nz * c->cfg.r;
-    unpack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(L, c->cfg.r, which ? c->Vz : c->Uz, d_out);
+    const long long tot = (long long)L.nx * L.ny * L.nz * c->rp;
+    unpack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(L, c->rp, which ? c->Vz : c->Uz, d_out);
     c->launches++;
     CU(cudaGetLastError());
     return RTM_OK;

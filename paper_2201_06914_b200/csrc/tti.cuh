@@ -22,7 +22,7 @@ constexpr int TTI_FX = TTI_TX + 16, TTI_FZ = TTI_TZ + 16;   // field tile (halo 
 constexpr int TTI_GX = TTI_TX + 8, TTI_GZ = TTI_TZ + 8;     // product tile (halo 4)
 constexpr int TTI_SMEM = (2 * TTI_FX * TTI_FZ + 4 * TTI_GX * TTI_GZ) * 4;
 
-template <int TM>
+template <int TM, bool TWO = false>
 __global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const StepArgs a) {
     extern __shared__ __align__(16) float smem[];
     float *sA = smem;                          // [FX][FZ]
@@ -214,7 +214,15 @@ __global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const St
             const long long o = (long long)ix * L.upz + iz;
             const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
             if (TM > 0) stcs4(a.hist + o, v);
-            else probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+            else if (!TWO) probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+            else {
+                // four compressed arrays for the TTI gradient (PAPER.md:L39-45 on the (p, r) system of L77; reading
+                // C29): p and r probed apart with the same row of Z, planes [0, r) and [r, 2r)
+                for (int f = 0; f < 2; f++) {
+                    const float4 w = f ? make_float4(rn[0], rn[1], rn[2], rn[3]) : make_float4(pn[0], pn[1], pn[2], pn[3]);
+                    probe_quad<2>(a.PZ + (long long)f * a.r * L.Nu + o, L.Nu, a.Zrow, a.r, w);
+                }
+            }
         }
     }
 }

@@ -323,3 +323,59 @@ def test_rademacher_probes():
     assert set(np.unique(p.Z)) == {-1.0, 1.0}
     for T in (0, 32):
         check_all(p, offsets=np.arange(-4, 5, dtype=np.int32), probe_block=T)
+
+
+@pytest.mark.parametrize("n,nt,r", [((75, 67), 77, 9), ((130, 41), 60, 4)])
+def test_tti_gradient_with_four_compressed_arrays(n, nt, r):
+    """SURVEY 8(f) item 1, reading C29: probe_fields = 2 probes p and r apart (Pz, Rz | Wpz, Wrz) with differenced
+    probes forward (Eq. 2-3 as printed) -- planes, image and gather against orc_propagate_pr; the propagation itself
+    is the one-field run's, bit for bit; r = nt identity probes against the sum over the stored (p, r) histories."""
+    import oracle as orc
+    from paper_2201_06914_b200 import Rtm, probes_dtt_host
+    p = ri.random_tti(n=n, nb=12, nt=nt, r=r, seed=33)
+    co = orc.coeffs(p)
+    one = run_gpu(p)
+    offs = np.array([-3, 0, 2], np.int32)
+    for Z in (p.Z, ri.identity_probes(p.nt)):
+        rr = Z.shape[1]
+        Zdd = probes_dtt_host(Z, p.dt)
+        m = Rtm.from_problem(p, r=rr, probe_fields=2)
+        m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        m.set_probes(Zdd, Z)
+        data = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz).cpu().numpy()
+        assert np.array_equal(data, one["data"])
+        img, q = m.adjoint_image(p.rec_xyz, data, p.src_xyz, qadj_out=True)
+        assert np.array_equal(q.cpu().numpy(), one["qadj"])
+        Uz, Vz = m.export_probes(0).cpu().numpy(), m.export_probes(1).cpu().numpy()
+        assert Uz.shape == (2 * rr, p.N)
+        img = img.cpu().numpy().ravel()
+        gat = m.offset_gather(offs).cpu().numpy().reshape(len(offs), -1)
+        m.close()
+        f = orc.forward(p, co, Z=Zdd, want_hist=True, fields=2)
+        a = orc.adjoint(p, co, data, Z=Z, want_hist=True, fields=2)
+        I = orc.image(f["PZ"], a["PZ"], 1.0 / rr)
+        G = orc.offset_gather(p.n, f["PZ"], a["PZ"], offs, 1.0 / rr)
+        errs = {"Pz": rel(Uz[:rr], f["PZ"][:rr]), "Rz": rel(Uz[rr:], f["PZ"][rr:]), "Wpz": rel(Vz[:rr], a["PZ"][:rr]),
+                "Wrz": rel(Vz[rr:], a["PZ"][rr:]), "image": rel(img, I), "gather": rel(gat, G)}
+        print(n, rr, {k: "%.2e" % v for k, v in errs.items()})
+        assert np.abs(I).max() > 0 and max(errs.values()) <= 1e-4, errs
+        assert np.array_equal(gat[1], img)                                       # PAPER.md:L52
+        assert rel(Uz[:rr], f["PZ"][rr:]) > 1e-3                                 # p and r planes are not swapped
+        if rr == p.nt:
+            Hp = np.concatenate([np.zeros((2,) + f["hist"].shape[1:]), f["hist"]])
+            D = (Hp[2:] - 2.0 * Hp[1:-1]) + Hp[:-2]
+            Iex = (D * a["hist"]).sum(axis=(0, 1)) / p.dt ** 2 * (float(Z[0, 0]) ** 2 / p.nt)
+            assert rel(img, Iex) <= 1e-4, rel(img, Iex)
+
+
+def test_four_array_mode_is_for_fused_tti_probing_only():
+    from paper_2201_06914_b200 import Rtm, RTMError
+    pa = ri.random_acoustic(2, n=(30, 28), nb=4, nt=10, r=2)
+    with pytest.raises(RTMError) as e:
+        Rtm.from_problem(pa, probe_fields=2)
+    assert e.value.code == -1
+    pt = ri.random_tti(n=(30, 28), nb=8, nt=10, r=2)
+    with pytest.raises(RTMError) as e:
+        Rtm.from_problem(pt, probe_fields=2, probe_block=8)
+    assert e.value.code == -1
+    Rtm.from_problem(pt, probe_fields=2, probe_block=1).close()
