@@ -94,6 +94,14 @@ int rtm_set_probes(rtm_ctx *ctx, const float *d_Zf, const float *d_Za, void *cud
  * to fp32.  h_Z, h_Zdd: HOST arrays [nt][r] (may not alias).  Errors: RTM_EINVAL.                      */
 int rtm_probes_dtt_host(int nt, int r, double dt, const float *h_Z, float *h_Zdd);
 
+/* Range-finder probes ("[Q, ~] = qr(A Z) where Z is a Rademacher random matrix"; refs [21, 26, 27];
+ * DESIGN.md reading C3): A = D D^T, the nt x nt temporal covariance of the shot record h_D [nt][nrec] the adjoint
+ * pass back-propagates (never formed); h_Q [nt][r] = orthonormal factor of the thin QR of D (D^T Z), diag(R) > 0.
+ * Q^T Q = I_r: pass h_Q to rtm_set_probes (upload it first) and use scale = 1.0f, not 1/r (u^T Q Q^T v is a
+ * projection).  Host pointers, fp64 arithmetic, one rounding to fp32.  Errors: RTM_EINVAL (r > nt, NULL, h_Q == h_Z,
+ * or D (D^T Z) numerically rank-deficient, e.g. r > rank D).                                                    */
+int rtm_probes_qr_host(int nt, int nrec, int r, const float *h_D, const float *h_Z, float *h_Q);
+
 /* Forward pass with fused probing (Eq. 3: u_bar = Z^T u accumulated on the fly).
  * Zeroes the wavefields and Uz, runs n = 0..nt-1:  time step with fused damping; inject
  * K2 h^(2-d) w wav[n][s] at the 2^d corners of each source; record d[n][j] = sum_c w u[corner];

@@ -173,6 +173,20 @@ def probes_dtt(Z, dt):
     return (((Zp[:nt] - 2.0 * Zp[1:nt + 1]) + Zp[2:nt + 2]) * (1.0 / (float(dt) * float(dt)))).astype(np.float32)
 
 
+def probes_qr(D, Z):
+    """PAPER.md:L33 "[Q, ~] = qr(A Z) where Z is a Rademacher random matrix": range-finder probes (refs [21, 26, 27]).
+    Reading C3: A = D D^T, the nt x nt temporal covariance of the shot record D [nt][nrec] that the
+    adjoint pass back-propagates (never formed: Y = D (D^T Z)); Q [nt][r] = the orthonormal factor of the thin QR of
+    Y with diag(R) > 0.  Q^T Q = I_r, so the estimator sum_k (Q^T u)_k (Q^T v)_k = u^T Q Q^T v is a projection and
+    its scale is 1, not 1/r.  fp64 (numpy.linalg.qr as the library step), one rounding to the fp32 the GPU receives."""
+    D = np.asarray(D, np.float32).astype(np.float64)
+    Z = np.asarray(Z, np.float32).astype(np.float64)
+    Y = D @ (D.T @ Z)
+    Q, R = np.linalg.qr(Y)
+    Q = Q * np.where(np.diag(R) < 0, -1.0, 1.0)[None, :]
+    return Q.astype(np.float32)
+
+
 def exact_gradient_image(uh, vh, dt):
     """Eq. 2 as printed: sum_t u_tt(t) v(t) from stored histories [nt][N], with the second time
     difference of the update itself, u_tt[n] = (w[n] - 2 w[n-1] + w[n-2]) / dt^2 (zero initial fields)."""

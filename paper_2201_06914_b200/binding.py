@@ -13,7 +13,7 @@ _LIBPATH = os.path.join(_HERE, "csrc", "librtm.so")
 _lib = None
 
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
-           "rtm_set_probes", "rtm_probes_dtt_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
+           "rtm_set_probes", "rtm_probes_dtt_host", "rtm_probes_qr_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
            "rtm_offset_gather_xy",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
            "rtm_export_coeff", "rtm_debug_stamps", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
@@ -55,6 +55,7 @@ def load_library():
     lib.rtm_set_model.argtypes = [vp] * 8
     lib.rtm_set_probes.argtypes = [vp] * 4
     lib.rtm_probes_dtt_host.argtypes = [ip, ip, C.c_double, vp, vp]
+    lib.rtm_probes_qr_host.argtypes = [ip, ip, ip, vp, vp, vp]
     lib.rtm_forward_probe.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp]
     lib.rtm_adjoint_image.argtypes = [vp, ip, vp, vp, ip, vp, vp, fp, ip, vp, vp]
     lib.rtm_offset_gather.argtypes = [vp, ip, vp, fp, vp, vp]
@@ -128,6 +129,16 @@ def coeffs_host(cfg: RtmConfig, vp, eps=None, delta=None, theta=None):
     _check(lib.rtm_coeffs_host(C.byref(cfg), _hp(vp), _hp(eps), _hp(delta), _hp(theta), _hp(K2),
                                _hp(outs[0]), _hp(outs[1]), _hp(outs[2]), _hp(outs[3]), _hp(damp)))
     return K2, outs[0], outs[1], outs[2], outs[3], damp
+
+
+def probes_qr_host(D, Z):
+    """rtm_probes_qr_host: Q [nt][r], orthonormal basis of range(D D^T Z); use with scale = 1."""
+    D = np.ascontiguousarray(D, np.float32)
+    Z = np.ascontiguousarray(Z, np.float32)
+    assert D.ndim == 2 and Z.ndim == 2 and D.shape[0] == Z.shape[0]
+    out = np.empty_like(Z)
+    _check(load_library().rtm_probes_qr_host(D.shape[0], D.shape[1], Z.shape[1], _hp(D), _hp(Z), _hp(out)))
+    return out
 
 
 def probes_dtt_host(Z, dt):

@@ -333,6 +333,45 @@ extern "C" int rtm_probes_dtt_host(int nt, int r, double dt, const float *h_Z, f
     return RTM_OK;
 }
 
+// ---- reading C3: range-finder probes [Q, ~] = qr(A Z), A = D D^T (host, fp64) -------------------
+// Y = D (D^T Z) without forming the nt x nt matrix, then Gram-Schmidt with one re-orthogonalisation pass per column
+// (the "twice is enough" variant: orthogonal to rounding for any Y that is not numerically rank-deficient).
+// Normalising by a positive norm gives the thin QR with diag(R) > 0, the unique one.
+extern "C" int rtm_probes_qr_host(int nt, int nrec, int r, const float *h_D, const float *h_Z, float *h_Q) {
+    if (nt < 1 || nrec < 1 || r < 1 || r > nt || !h_D || !h_Z || !h_Q || h_Z == h_Q) return RTM_EINVAL;
+    std::vector<double> W((size_t)nrec * r, 0.0), Y((size_t)r * nt, 0.0);   // W = D^T Z [nrec][r]; Y column-major [r][nt]
+    for (int n = 0; n < nt; n++)
+        for (int j = 0; j < nrec; j++) {
+            const double d = h_D[(size_t)n * nrec + j];
+            for (int k = 0; k < r; k++) W[(size_t)j * r + k] += d * (double)h_Z[(size_t)n * r + k];
+        }
+    for (int n = 0; n < nt; n++)
+        for (int j = 0; j < nrec; j++) {
+            const double d = h_D[(size_t)n * nrec + j];
+            for (int k = 0; k < r; k++) Y[(size_t)k * nt + n] += d * W[(size_t)j * r + k];
+        }
+    for (int k = 0; k < r; k++) {
+        double *y = &Y[(size_t)k * nt];
+        double n0 = 0.0;
+        for (int n = 0; n < nt; n++) n0 += y[n] * y[n];
+        for (int pass = 0; pass < 2; pass++)
+            for (int i = 0; i < k; i++) {
+                const double *q = &Y[(size_t)i * nt];
+                double dot = 0.0;
+                for (int n = 0; n < nt; n++) dot += q[n] * y[n];
+                for (int n = 0; n < nt; n++) y[n] -= dot * q[n];
+            }
+        double n1 = 0.0;
+        for (int n = 0; n < nt; n++) n1 += y[n] * y[n];
+        if (!(n1 > 1e-24 * n0) || !(n0 > 0.0)) return RTM_EINVAL;   // A Z is numerically rank-deficient (r > rank D)
+        const double inv = 1.0 / std::sqrt(n1);
+        for (int n = 0; n < nt; n++) y[n] *= inv;
+    }
+    for (int n = 0; n < nt; n++)
+        for (int k = 0; k < r; k++) h_Q[(size_t)n * r + k] = (float)Y[(size_t)k * nt + n];
+    return RTM_OK;
+}
+
 static int launch_pack(rtm_ctx *c, const float *src, float *dst, cudaStream_t st) {
     const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pz;
     pack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, st>>>(c->L, src, dst);

@@ -4,6 +4,7 @@ import os
 import re
 
 import numpy as np
+import pytest
 
 import oracle as orc
 import rtm_inputs as ri
@@ -90,3 +91,27 @@ def test_host_coefficients_match_oracle_bitwise():
         if p.physics == 1:
             for a, b in ((eh, co.epsh), (dh, co.delh), (cs, co.cosT), (sn, co.sinT)):
                 assert np.array_equal(a, b)
+
+
+def test_qr_probes_host_match_oracle():
+    """rtm_probes_qr_host (Gram-Schmidt with re-orthogonalisation, host fp64; no GPU needed) against the oracle's
+    numpy.linalg.qr: the thin QR with diag(R) > 0 is unique, so Q itself is compared (reading C3), plus the projector
+    and the error paths."""
+    import oracle as orc
+    import rtm_inputs as ri
+    from paper_2201_06914_b200 import RTMError, probes_qr_host
+    rng = np.random.default_rng(3)
+    for nt, nrec, r in ((96, 40, 8), (61, 7, 5), (33, 50, 33)):
+        D = rng.standard_normal((nt, nrec)).astype(np.float32) * np.linspace(1.0, 0.05, nrec, dtype=np.float32)
+        Z = ri.rademacher_probes(nt, r, seed=nt)
+        Q = probes_qr_host(D, Z)
+        ref = orc.probes_qr(D, Z)
+        assert np.abs(Q.astype(np.float64) - ref).max() <= 2e-6, (nt, nrec, r, np.abs(Q - ref).max())
+        Q64 = Q.astype(np.float64)
+        assert np.abs(Q64.T @ Q64 - np.eye(r)).max() <= 1e-6
+    with pytest.raises(RTMError) as e:                       # r > rank D: D (D^T Z) is rank-deficient
+        probes_qr_host(rng.standard_normal((20, 3)).astype(np.float32), ri.rademacher_probes(20, 5, seed=1))
+    assert e.value.code == -1
+    with pytest.raises(RTMError) as e:                       # r > nt
+        probes_qr_host(rng.standard_normal((4, 9)).astype(np.float32), np.ones((4, 6), np.float32))
+    assert e.value.code == -1

@@ -379,3 +379,34 @@ def test_four_array_mode_is_for_fused_tti_probing_only():
         Rtm.from_problem(pt, probe_fields=2, probe_block=8)
     assert e.value.code == -1
     Rtm.from_problem(pt, probe_fields=2, probe_block=1).close()
+
+
+def test_qr_range_finder_probes():
+    """PAPER.md:L33, reading C3: Q = rtm_probes_qr_host(record, Rademacher Z) as probes, scale 1: compressed
+    wavefields and image against the oracle fed with its own probes_qr; on this cropped c0 the r = 8 image is within
+    5 % of sum_t u v from the oracle's stored histories."""
+    import oracle as orc
+    from paper_2201_06914_b200 import Rtm, probes_qr_host
+    p = ri.make_c0(nt=200, r=8, n=(41, 41), nb=12)
+    co = orc.coeffs(p)
+    f0 = orc.forward(p, co, want_hist=True)
+    din = f0["samples"].astype(np.float32)
+    Zr = ri.rademacher_probes(p.nt, p.r, seed=3)
+    Q = probes_qr_host(din, Zr)
+    Qo = orc.probes_qr(din, Zr)
+    assert np.abs(Q - Qo).max() <= 2e-6
+    m = Rtm.from_problem(p)
+    m.set_model_from_earth(p.vp)
+    m.set_probes(Q)
+    m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    img, _ = m.adjoint_image(p.rec_xyz, din, p.src_xyz, scale=1.0)
+    Uz, Vz = m.export_probes(0).cpu().numpy(), m.export_probes(1).cpu().numpy()
+    img = img.cpu().numpy().ravel()
+    m.close()
+    f = orc.forward(p, co, Z=Qo)
+    a = orc.adjoint(p, co, din, Z=Qo, want_hist=True)
+    I = orc.image(f["PZ"], a["PZ"], 1.0)
+    # Q differs from Qo by fp64 rounding before the fp32 rounding: a few entries may land one ulp apart
+    assert rel(Uz, f["PZ"]) <= 1e-4 and rel(Vz, a["PZ"]) <= 1e-4 and rel(img, I) <= 1e-4
+    Iex = orc.exact_image(f0["hist"], a["hist"])
+    assert rel(img, Iex) <= 0.05, rel(img, Iex)
