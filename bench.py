@@ -310,6 +310,15 @@ def run_ours(args):
     if offs is not None:
         gather_ms = timed(lambda: m.offset_gather(offs, out=gather), 10) / 10
 
+    # ---- (hx, hy) offset volume on 3D grids (reading C28): 9 x 3 offsets, three tiled launches -----
+    gxy_ms, gxy_offs = None, None
+    if p.ndim == 3:
+        gxy_offs = np.array([(hx, hy) for hy in (-1, 0, 1) for hx in range(-4, 5)], np.int32)
+        gxy = torch.empty((len(gxy_offs),) + tuple(p.n), dtype=torch.float32, device=dev)
+        m.offset_gather_xy(gxy_offs, out=gxy)
+        gxy_ms = timed(lambda: m.offset_gather_xy(gxy_offs, out=gxy), 3) / 3
+        del gxy
+
     # ---- end to end: host buffers through rtm_shot_host ------------------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_wav, h_din = pin(p.wav), din.cpu().pin_memory()
@@ -391,6 +400,12 @@ def run_ours(args):
             out["gather"] = {"kernel": "gather_tiled_kernel", "nh": int(len(offs)), "ms": gather_ms,
                              "min_bytes": gb, "achieved": gb / (gather_ms * 1e-3) / 1e9, "unit": "GB/s",
                              "frac": gb / (gather_ms * 1e-3) / 1e9 / peak}
+        if gxy_ms is not None:
+            # per tiled launch: Uz and Vz read once, 9 offset planes written once
+            gb = 3 * 8.0 * p.r * p.N + 4.0 * len(gxy_offs) * p.N
+            out["gather_xy"] = {"kernel": "gather_tiled_kernel<16>", "offsets": "hx -4..4 x hy -1..1", "launches": 3,
+                                "ms": gxy_ms, "min_bytes": gb, "achieved": gb / (gxy_ms * 1e-3) / 1e9, "unit": "GB/s",
+                                "frac": gb / (gxy_ms * 1e-3) / 1e9 / peak}
         if other is not None:
             T2, ms2, f2, a2 = other
             out["variant"] = {"probe": "per-step fused" if T2 <= 1 else "time-blocked, T=%d" % T2,

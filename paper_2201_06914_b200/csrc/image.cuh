@@ -115,25 +115,34 @@ __global__ void __launch_bounds__(256) gather_xy_kernel(Layout L, const float *_
 // a thread then reads 15 + 15 values and does 64 FMAs: acc[i][j] += U[i + j] * V[i - j + 7].
 // Same products in the same order (k ascending, one fma each) as the generic kernel and as image_kernel, so
 // gather[h = 0] stays bit-identical to the image.
-constexpr int GT_X = 32, GT_HP = 48, GT_ROWS = GT_X + GT_HP - 1, GT_THREADS = 32 * (GT_X / 8) * (GT_HP / 8);
-constexpr int GT_SMEM = 2 * 2 * GT_ROWS * 32 * 4;
+// HP = offsets per launch: 48 (c3's 41 offsets in one launch) or 16 (the short hx runs of (hx, hy) volumes: 47 instead
+// of 79 staged rows per tile, 8 warps instead of 24).
+constexpr int GT_X = 32, GT_HP = 48;
+__host__ __device__ constexpr int gt_rows(int hp) { return GT_X + hp - 1; }
+__host__ __device__ constexpr int gt_threads(int hp) { return 32 * (GT_X / 8) * (hp / 8); }
+__host__ __device__ constexpr int gt_smem(int hp) { return 2 * 2 * gt_rows(hp) * 32 * 4; }
 
-__global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, const float *__restrict__ U,
+template <int HP, bool XY>
+__global__ void __launch_bounds__(gt_threads(HP)) gather_tiled_kernel(Layout L, const float *__restrict__ U,
                                                                    const float *__restrict__ V, int r, int nh, int h0,
                                                                    int hy, float scale, float *__restrict__ G) {
+    constexpr int GT_ROWS = gt_rows(HP), GT_THREADS = gt_threads(HP);
     extern __shared__ __align__(16) float gsm[];   // [2 buffers][U | V][GT_ROWS][32]
     const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
     const int xg = grp % (GT_X / 8), hg = grp / (GT_X / 8);
     const long long R = (long long)L.ny * L.upz;
     const long long l0 = (long long)blockIdx.x * 32;          // first float of the fast axes
     const int x0 = blockIdx.y * GT_X;
-    const int xu0 = x0 + h0, xv0 = x0 - (h0 + GT_HP - 1);     // first x row of the U / V tile
+    const int xu0 = x0 + h0, xv0 = x0 - (h0 + HP - 1);     // first x row of the U / V tile
     // vector offsets (hx, hy) on 3D grids (reading C28): upz % 32 == 0, so the block's 32 floats lie in one y row
     // iy0 and a shift by hy along y is a shift by hy * upz floats, valid for the whole block or for none of it
-    const int iy0 = (int)(l0 / L.upz);
-    const bool yok = iy0 + hy >= 0 && iy0 + hy < L.ny && iy0 - hy >= 0 && iy0 - hy < L.ny;
-    const long long lu = l0 + (long long)(yok ? hy : 0) * L.upz, lv = l0 - (long long)(yok ? hy : 0) * L.upz;
-    const bool active = hg * 8 < nh;                           // offset groups beyond nh only help with the staging
+    if (XY) {
+        const int iy0 = (int)(l0 / L.upz);
+        const bool yok = iy0 + hy >= 0 && iy0 + hy < L.ny && iy0 - hy >= 0 && iy0 - hy < L.ny;
+        if (!yok) r = 0;                                       // every term vanishes (C28): the block writes zeros
+        U += (long long)hy * L.upz;
+        V -= (long long)hy * L.upz;
+    }
 
     auto request = [&](int k, int buf) {
         float *dst = gsm + buf * (2 * GT_ROWS * 32);
@@ -142,8 +151,8 @@ __global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, cons
             const int row = c >> 3, q = c & 7;
             const bool isV = row >= GT_ROWS;
             const int x = isV ? xv0 + (row - GT_ROWS) : xu0 + row;
-            const bool ok = yok && x >= 0 && x < L.nx;
-            const float *src = (isV ? V : U) + (long long)k * L.Nu + (long long)(ok ? x : 0) * R + (isV ? lv : lu) + q * 4;
+            const bool ok = x >= 0 && x < L.nx;
+            const float *src = (isV ? V : U) + (long long)k * L.Nu + (long long)(ok ? x : 0) * R + l0 + q * 4;
             cp_async16(dst + row * 32 + q * 4, src, ok);
         }
         cp_async_commit();
@@ -155,14 +164,13 @@ __global__ void __launch_bounds__(GT_THREADS) gather_tiled_kernel(Layout L, cons
 #pragma unroll
         for (int j = 0; j < 8; j++) acc[i][j] = 0.f;
 
-    request(0, 0);
+    if (!XY || r > 0) request(0, 0);
     for (int k = 0; k < r; k++) {
         cp_async_wait<0>();
         __syncthreads();            // probe k has landed for everybody; nobody still reads the other buffer
         if (k + 1 < r) request(k + 1, (k + 1) & 1);
-        if (!active) continue;
         const float *us = gsm + (k & 1) * (2 * GT_ROWS * 32) + (8 * (xg + hg)) * 32 + lane;
-        const float *vs = gsm + (k & 1) * (2 * GT_ROWS * 32) + (GT_ROWS + 8 * xg - 8 * hg + GT_HP - 8) * 32 + lane;
+        const float *vs = gsm + (k & 1) * (2 * GT_ROWS * 32) + (GT_ROWS + 8 * xg - 8 * hg + HP - 8) * 32 + lane;
         float u[15], v[15];
 #pragma unroll
         for (int m = 0; m < 15; m++) { u[m] = us[m * 32]; v[m] = vs[m * 32]; }

@@ -843,7 +843,8 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
     for (int i = 1; i < nh && run; i++) run = h_offsets[i] == h_offsets[i - 1] + 1;
     if (run) {
         const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
-        gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], 0, scale, d_gather);
+        if (nh <= 16) gather_tiled_kernel<16, false><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], 0, scale, d_gather);
+        else gather_tiled_kernel<GT_HP, false><<<grid, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], 0, scale, d_gather);
     } else {
         const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
         gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->rp, nh, c->offs, scale, d_gather);
@@ -871,8 +872,12 @@ extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy,
             j++;
         if (j - i >= 8) {
             const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
-            gather_tiled_kernel<<<grid, GT_THREADS, GT_SMEM, st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
-                                                                   h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
+            if (j - i <= 16)
+                gather_tiled_kernel<16, true><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
+                                                                                   h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
+            else
+                gather_tiled_kernel<GT_HP, true><<<grid, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
+                                                                                            h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
             c->launches++;
         } else {
             for (int m = i; m < j; m++) {
