@@ -50,7 +50,9 @@ struct StepArgs {
     float *PZ;
     const float *Zrow;
     int r;
-    int two;                // TTI, probe_fields = 2 (reading C29): p -> planes [0, r), r -> planes [r, 2r) of PZ
+    int two;                // TTI, probe_fields = 2 (reading C29): plane 2k of PZ = probe k of p, plane 2k + 1 = probe k of r
+    long long pNu;          // floats per probe-plane group and per history slot: Nu, or 2 Nu with two probed fields (the
+                            // r field then sits Nu floats behind the p field: to the flush roles it is nx more rows)
     // time-blocked probing: instead of PZ, store the probed field into this history slot (physical grid,
     // probe-plane layout); probe_flush_kernel applies T rows of Z at once
     float *hist;
@@ -187,7 +189,7 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
         const long long o = row * L.upz + iz;
         float2 h[TM];
 #pragma unroll
-        for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs2(a.fl_hist + j * L.Nu + o) : make_float2(0.f, 0.f);
+        for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs2(a.fl_hist + j * a.pNu + o) : make_float2(0.f, 0.f);
         float *p = a.PZ + o;
         // software-pipelined over groups of 4 planes, DEPTH groups in flight: the loads of later groups are issued
         // BEFORE the stores of the current one (the compiler cannot hoist them itself: it cannot prove the planes do
@@ -199,7 +201,7 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
         for (int s = 0; s < DEPTH; s++)
 #pragma unroll
             for (int i = 0; i < G; i++)
-                ring[s][i] = (s * G + i < r) ? ldcs2(p + (long long)(s * G + i) * L.Nu) : make_float2(0.f, 0.f);
+                ring[s][i] = (s * G + i < r) ? ldcs2(p + (long long)(s * G + i) * a.pNu) : make_float2(0.f, 0.f);
         for (int kk = 0; kk < r; kk += G * DEPTH) {   // Z rows are zero-padded to zr (multiple of 8)
 #pragma unroll
             for (int s = 0; s < DEPTH; s++) {
@@ -211,7 +213,7 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
 #pragma unroll
                 for (int i = 0; i < G; i++) {
                     const int kn = k + G * DEPTH + i;
-                    ring[s][i] = (kn < r) ? ldcs2(p + (long long)kn * L.Nu) : make_float2(0.f, 0.f);
+                    ring[s][i] = (kn < r) ? ldcs2(p + (long long)kn * a.pNu) : make_float2(0.f, 0.f);
                 }
 #pragma unroll
                 for (int j = 0; j < TM; j++) {
@@ -223,7 +225,7 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
                 }
 #pragma unroll
                 for (int i = 0; i < G; i++)
-                    if (k + i < r) stcs2(p + (long long)(k + i) * L.Nu, acc[i]);
+                    if (k + i < r) stcs2(p + (long long)(k + i) * a.pNu, acc[i]);
             }
         }
     }
@@ -253,7 +255,7 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
         const long long o = row * L.upz + iz;
         float4 h[TM];
 #pragma unroll
-        for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs4(a.fl_hist + j * L.Nu + o) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int j = 0; j < TM; j++) h[j] = j < n ? ldcs4(a.fl_hist + j * a.pNu + o) : make_float4(0.f, 0.f, 0.f, 0.f);
         float *p = a.PZ + o;
         // The plane loop is a chain of DRAM round trips (load - FMA - store per group): with one group of look-ahead
         // the role needed 1 + r/2 round trips per thread (measured 15 us at c1, longer than the stencil blocks it
@@ -264,7 +266,7 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
         for (int s = 0; s < DEPTH; s++)
 #pragma unroll
             for (int i = 0; i < G; i++)
-                ring[s][i] = (s * G + i < r) ? ldcs4(p + (long long)(s * G + i) * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+                ring[s][i] = (s * G + i < r) ? ldcs4(p + (long long)(s * G + i) * a.pNu) : make_float4(0.f, 0.f, 0.f, 0.f);
         for (int kk = 0; kk < r; kk += G * DEPTH) {   // Z rows are zero-padded to zr (multiple of 8)
 #pragma unroll
             for (int s = 0; s < DEPTH; s++) {
@@ -276,7 +278,7 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
 #pragma unroll
                 for (int i = 0; i < G; i++) {
                     const int kn = k + G * DEPTH + i;
-                    ring[s][i] = (kn < r) ? ldcs4(p + (long long)kn * L.Nu) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    ring[s][i] = (kn < r) ? ldcs4(p + (long long)kn * a.pNu) : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
 #pragma unroll
                 for (int j = 0; j < TM; j++) {
@@ -288,7 +290,7 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
                 }
 #pragma unroll
                 for (int i = 0; i < G; i++)
-                    if (k + i < r) stcs4(p + (long long)(k + i) * L.Nu, acc[i]);
+                    if (k + i < r) stcs4(p + (long long)(k + i) * a.pNu, acc[i]);
             }
         }
     }

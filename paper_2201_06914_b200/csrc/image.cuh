@@ -120,19 +120,23 @@ __global__ void __launch_bounds__(256) gather_xy_kernel(Layout L, const float *_
 constexpr int GT_X = 32, GT_HP = 48;
 __host__ __device__ constexpr int gt_rows(int hp) { return GT_X + hp - 1; }
 __host__ __device__ constexpr int gt_threads(int hp) { return 32 * (GT_X / 8) * (hp / 8); }
-__host__ __device__ constexpr int gt_smem(int hp) { return 2 * 2 * gt_rows(hp) * 32 * 4; }
+__host__ __device__ constexpr int gt_stages(int hp) { return hp <= 16 ? 4 : 2; }   // probes in flight (shared-memory buffers)
+__host__ __device__ constexpr int gt_smem(int hp) { return gt_stages(hp) * 2 * gt_rows(hp) * 32 * 4; }
 
 template <int HP, bool XY>
 __global__ void __launch_bounds__(gt_threads(HP)) gather_tiled_kernel(Layout L, const float *__restrict__ U,
                                                                    const float *__restrict__ V, int r, int nh, int h0,
                                                                    int hy, float scale, float *__restrict__ G) {
-    constexpr int GT_ROWS = gt_rows(HP), GT_THREADS = gt_threads(HP);
-    extern __shared__ __align__(16) float gsm[];   // [2 buffers][U | V][GT_ROWS][32]
+    constexpr int GT_ROWS = gt_rows(HP), GT_THREADS = gt_threads(HP), NST = gt_stages(HP);
+    extern __shared__ __align__(16) float gsm[];   // [NST buffers][U | V][GT_ROWS][32]
     const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
     const int xg = grp % (GT_X / 8), hg = grp / (GT_X / 8);
     const long long R = (long long)L.ny * L.upz;
-    const long long l0 = (long long)blockIdx.x * 32;          // first float of the fast axes
-    const int x0 = blockIdx.y * GT_X;
+    // 1-D offsets: grid (l blocks, x tiles).  (hx, hy) volumes: 1-D grid with the x tiles fastest, so that the blocks
+    // sharing halo rows run together and the re-read rows come from L2 (ncu, c4: 1.43x the minimum from DRAM otherwise)
+    const int nxt = (L.nx + GT_X - 1) / GT_X;
+    const long long l0 = (long long)(XY ? blockIdx.x / nxt : blockIdx.x) * 32;   // first float of the fast axes
+    const int x0 = (XY ? blockIdx.x % nxt : blockIdx.y) * GT_X;
     const int xu0 = x0 + h0, xv0 = x0 - (h0 + HP - 1);     // first x row of the U / V tile
     // vector offsets (hx, hy) on 3D grids (reading C28): upz % 32 == 0, so the block's 32 floats lie in one y row
     // iy0 and a shift by hy along y is a shift by hy * upz floats, valid for the whole block or for none of it
@@ -164,13 +168,19 @@ __global__ void __launch_bounds__(gt_threads(HP)) gather_tiled_kernel(Layout L, 
 #pragma unroll
         for (int j = 0; j < 8; j++) acc[i][j] = 0.f;
 
-    if (!XY || r > 0) request(0, 0);
+    // NST - 1 probes in flight ahead of the one being consumed; one commit group per probe slot (empty past the end)
+#pragma unroll
+    for (int q = 0; q < NST - 1; q++) {
+        if (q < r) request(q, q);
+        else cp_async_commit();
+    }
     for (int k = 0; k < r; k++) {
-        cp_async_wait<0>();
-        __syncthreads();            // probe k has landed for everybody; nobody still reads the other buffer
-        if (k + 1 < r) request(k + 1, (k + 1) & 1);
-        const float *us = gsm + (k & 1) * (2 * GT_ROWS * 32) + (8 * (xg + hg)) * 32 + lane;
-        const float *vs = gsm + (k & 1) * (2 * GT_ROWS * 32) + (GT_ROWS + 8 * xg - 8 * hg + HP - 8) * 32 + lane;
+        cp_async_wait<NST - 2>();
+        __syncthreads();            // probe k has landed for everybody; nobody still reads the buffer of probe k - 1
+        if (k + NST - 1 < r) request(k + NST - 1, (k + NST - 1) % NST);
+        else cp_async_commit();
+        const float *us = gsm + (k % NST) * (2 * GT_ROWS * 32) + (8 * (xg + hg)) * 32 + lane;
+        const float *vs = gsm + (k % NST) * (2 * GT_ROWS * 32) + (GT_ROWS + 8 * xg - 8 * hg + HP - 8) * 32 + lane;
         float u[15], v[15];
 #pragma unroll
         for (int m = 0; m < 15; m++) { u[m] = us[m * 32]; v[m] = vs[m * 32]; }
@@ -217,11 +227,13 @@ __global__ void unpack_field_kernel(Layout L, const float *__restrict__ src, flo
     dst[t] = src[L.org + jx * L.sx + jy * L.sy + jz];
 }
 // internal probe planes -> canonical [r][N]
-__global__ void unpack_probes_kernel(Layout L, int r, const float *__restrict__ src, float *__restrict__ dst) {
+// two != 0 (probe_fields = 2): r counts all 2 r_probes planes; canonical plane f r_probes + k = internal plane 2k + f
+__global__ void unpack_probes_kernel(Layout L, int r, int two, const float *__restrict__ src, float *__restrict__ dst) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long N = (long long)L.nx * L.ny * L.nz;
     if (t >= N * r) return;
-    const int k = (int)(t / N);
+    int k = (int)(t / N);
+    if (two) { const int rh = r / 2; k = k < rh ? 2 * k : 2 * (k - rh) + 1; }
     const long long x = t % N;
     const int iz = (int)(x % L.nz);
     const long long row = x / L.nz;

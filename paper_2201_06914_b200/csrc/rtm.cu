@@ -55,6 +55,7 @@ struct rtm_ctx {
     float *k1x, *k1y, *k1z;
     float *Uz, *Vz, *Zf, *Za, *hist;
     int zr, T, rx;
+    long long pNu;   // floats per history slot and per group of planes of one probe: Nu x probed fields
     int rp;   // probe planes per compressed array: r, or 2 r when p and r are probed apart (probe_fields = 2)
     int *row_start;
     InjEntry *ent;
@@ -95,9 +96,9 @@ static bool valid_cfg(const rtm_config *c) {
     // flush-role thread, the TTI kernel (64 registers) has not
     if (c->probe_block < 0 || c->probe_block > (c->physics == 0 ? 32 : 16)) return false;
     if (c->probe_block > 16 && c->r > 128) return false;   // staging of the 32 Z rows in the final flush kernel
-    // four compressed arrays for the TTI gradient (reading C29): TTI with the probe fused into every step only
+    // four compressed arrays for the TTI gradient (reading C29): TTI only
     if (c->probe_fields != 0 && c->probe_fields != 1 && c->probe_fields != 2) return false;
-    if (c->probe_fields == 2 && (c->physics != 1 || c->probe_block > 1)) return false;
+    if (c->probe_fields == 2 && c->physics != 1) return false;
     return true;
 }
 
@@ -146,7 +147,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t pb = (size_t)rp * (size_t)L.Nu * 4;
     size_t o_U = take(pb), o_V = take(pb);
     const int T = c->probe_block > 1 ? c->probe_block : 0;
-    size_t o_H = take(2 * (size_t)T * (size_t)L.Nu * 4);   // double-buffered history ring
+    size_t o_H = take(2 * (size_t)T * (size_t)(rp / c->r) * (size_t)L.Nu * 4);   // double-buffered history ring (per probed field)
     const int zr = (int)rup(c->r, 8);
     size_t zb = (size_t)c->nt * zr * 4;
     size_t o_Zf = take(zb), o_Za = take(zb);
@@ -183,6 +184,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->Za = (float *)(b + o_Za);
         ctx->zr = zr;
         ctx->rp = rp;
+        ctx->pNu = (long long)(rp / c->r) * L.Nu;
         ctx->row_start = (int *)(b + o_rs);
         ctx->ent = (InjEntry *)(b + o_en);
         ctx->smp_idx = (int *)(b + o_si);
@@ -632,9 +634,12 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
         switch (tm) {
             case 0: return a.two ? launch_ex(c, tti_step_kernel<0, true>, a, nb, block, smem, st)
                                  : launch_ex(c, tti_step_kernel<0>, a, nb, block, smem, st);
-            case 4: return launch_ex(c, tti_step_kernel<4>, a, nb, block, smem, st);
-            case 8: return launch_ex(c, tti_step_kernel<8>, a, nb, block, smem, st);
-            default: return launch_ex(c, tti_step_kernel<16>, a, nb, block, smem, st);
+            case 4: return a.two ? launch_ex(c, tti_step_kernel<4, true>, a, nb, block, smem, st)
+                                 : launch_ex(c, tti_step_kernel<4>, a, nb, block, smem, st);
+            case 8: return a.two ? launch_ex(c, tti_step_kernel<8, true>, a, nb, block, smem, st)
+                                 : launch_ex(c, tti_step_kernel<8>, a, nb, block, smem, st);
+            default: return a.two ? launch_ex(c, tti_step_kernel<16, true>, a, nb, block, smem, st)
+                                  : launch_ex(c, tti_step_kernel<16>, a, nb, block, smem, st);
         }
     } else if (c->cfg.ndim == 2) {
         switch (tm) {
@@ -657,7 +662,10 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
 }
 
 static int launch_flush(rtm_ctx *c, const float *hist, int ncur, const float *Z0, long long zstep, float *PZ, cudaStream_t st) {
-    const Layout &L = c->L;
+    // two probed fields: the r field sits Nu floats behind the p field in every slot and plane group, i.e. it is nx more
+    // rows of the same pitch
+    Layout L = c->L;
+    if (c->cfg.probe_fields == 2) { L.nx *= 2; L.Nu *= 2; }
     const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
     const unsigned nb = (unsigned)((tot + 255) / 256);
     if (c->T <= 4) probe_flush_kernel<4><<<nb, 256, 0, st>>>(L, hist, ncur, Z0, zstep, c->zr, c->cfg.r, PZ);
@@ -686,6 +694,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     a.PZ = PZ;
     a.r = cfg.r;
     a.two = cfg.probe_fields == 2;
+    a.pNu = c->pNu;
     a.row_start = c->row_start;
     a.ent = c->ent;
     double inj_scale = adjoint ? (double)cfg.h * (double)cfg.h : std::pow((double)cfg.h, 2.0 - d);
@@ -705,7 +714,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     const long long nblocks = (long long)grid.x * grid.y * grid.z;
     const long long bthreads = (long long)block.x * block.y * block.z;
     const int fl_vec = (c->rx && T <= 16) ? 4 : 2;   // floats per flush-role thread (flush_role4 in the 2D streaming kernel)
-    const long long units = (long long)L.nx * L.ny * (L.upz / fl_vec);
+    const long long units = (long long)L.nx * L.ny * (L.upz / fl_vec) * (a.two ? 2 : 1);
     a.gx = grid.x; a.gy = grid.y;
     if (c->rx) a.gx = (unsigned)((L.Pz + 3) / 4);   // streaming kernel: quads per row
     a.zr = c->zr;
@@ -731,12 +740,12 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
             // time block b = step / T writes history slots [(b&1) T, (b&1) T + T); while it runs, the
             // previous block is flushed in len_b slices, one per step launch
             const int b = step / T, slot = step % T;
-            a.hist = c->hist + ((size_t)(b & 1) * T + slot) * L.Nu;
+            a.hist = c->hist + ((size_t)(b & 1) * T + slot) * c->pNu;
             if (b >= 1) {
                 const int len_b = std::min(T, nt - b * T);
                 const int pb = b - 1;
                 const int nfirst = adjoint ? nt - 1 - pb * T : pb * T;
-                a.fl_hist = c->hist + (size_t)(pb & 1) * T * L.Nu;
+                a.fl_hist = c->hist + (size_t)(pb & 1) * T * c->pNu;
                 a.fl_Z0 = Z + (size_t)nfirst * c->zr;
                 a.fl_n = T;
                 // slices go to slots 1 .. len_b-1: their input (the previous block's last slot) is then at least two
@@ -758,7 +767,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
         if (T && step == nt - 1) {   // the last time block has no following steps to hide behind
             const int fb = step / T, lenf = nt - fb * T;
             const int nfirst = adjoint ? nt - 1 - fb * T : fb * T;
-            launch_flush(c, c->hist + (size_t)(fb & 1) * T * L.Nu, lenf, Z + (size_t)nfirst * c->zr, a.fl_zstep, PZ, st);
+            launch_flush(c, c->hist + (size_t)(fb & 1) * T * c->pNu, lenf, Z + (size_t)nfirst * c->zr, a.fl_zstep, PZ, st);
         }
         if (c->opt_time && step == nt - 1) { CU(cudaEventRecord(c->ev[adjoint][1], st)); c->ev_valid[adjoint] = true; }
         if (want_smp && (!deferred || step == nt - 1)) {
@@ -871,7 +880,9 @@ extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy,
                h_offsets_xy[2 * j] == h_offsets_xy[2 * (j - 1)] + 1)
             j++;
         if (j - i >= 8) {
-            const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
+            const long long nblk = (((long long)L.ny * L.upz) / 32) * ((L.nx + GT_X - 1) / GT_X);   // x tiles fastest
+            if (nblk >= (1LL << 31)) return RTM_EINVAL;
+            const dim3 grid((unsigned)nblk, 1, 1);
             if (j - i <= 16)
                 gather_tiled_kernel<16, true><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
                                                                                    h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
@@ -953,7 +964,7 @@ extern "C" int rtm_export_probes(rtm_ctx *c, int which, float *d_out, void *stre
     if (which == 0 ? !c->have_U : !c->have_V) return RTM_ESTATE;
     const Layout &L = c->L;
     const long long tot = (long long)L.nx * L.ny * L.nz * c->rp;
-    unpack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(L, c->rp, which ? c->Vz : c->Uz, d_out);
+    unpack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(L, c->rp, c->cfg.probe_fields == 2, which ? c->Vz : c->Uz, d_out);
     c->launches++;
     CU(cudaGetLastError());
     return RTM_OK;

@@ -213,14 +213,19 @@ __global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const St
         if (ix >= 0 && ix < L.nx && iz >= 0 && iz < L.nz) {
             const long long o = (long long)ix * L.upz + iz;
             const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
-            if (TM > 0) stcs4(a.hist + o, v);
-            else if (!TWO) probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
-            else {
+            if (!TWO) {
+                if (TM > 0) stcs4(a.hist + o, v);
+                else probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+            } else {
                 // four compressed arrays for the TTI gradient (PAPER.md:L39-45 on the (p, r) system of L77; reading
-                // C29): p and r probed apart with the same row of Z, planes [0, r) and [r, 2r)
-                for (int f = 0; f < 2; f++) {
-                    const float4 w = f ? make_float4(rn[0], rn[1], rn[2], rn[3]) : make_float4(pn[0], pn[1], pn[2], pn[3]);
-                    probe_quad<2>(a.PZ + (long long)f * a.r * L.Nu + o, L.Nu, a.Zrow, a.r, w);
+                // C29): p and r probed apart with the same row of Z; plane (or history half-slot) 2k = p, 2k + 1 = r
+                const float4 wp = make_float4(pn[0], pn[1], pn[2], pn[3]), wr = make_float4(rn[0], rn[1], rn[2], rn[3]);
+                if (TM > 0) {
+                    stcs4(a.hist + o, wp);
+                    stcs4(a.hist + L.Nu + o, wr);
+                } else {
+                    for (int f = 0; f < 2; f++)
+                        probe_quad<2>(a.PZ + (long long)f * L.Nu + o, 2 * L.Nu, a.Zrow, a.r, f ? wr : wp);
                 }
             }
         }

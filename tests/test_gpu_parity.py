@@ -325,21 +325,23 @@ def test_rademacher_probes():
         check_all(p, offsets=np.arange(-4, 5, dtype=np.int32), probe_block=T)
 
 
-@pytest.mark.parametrize("n,nt,r", [((75, 67), 77, 9), ((130, 41), 60, 4)])
-def test_tti_gradient_with_four_compressed_arrays(n, nt, r):
+@pytest.mark.parametrize("n,nt,r,T", [((75, 67), 77, 9, 0), ((130, 41), 60, 4, 0), ((75, 67), 77, 9, 16), ((130, 41), 60, 4, 8),
+                                      ((33, 150), 50, 3, 4)])
+def test_tti_gradient_with_four_compressed_arrays(n, nt, r, T):
     """SURVEY 8(f) item 1, reading C29: probe_fields = 2 probes p and r apart (Pz, Rz | Wpz, Wrz) with differenced
     probes forward (Eq. 2-3 as printed) -- planes, image and gather against orc_propagate_pr; the propagation itself
-    is the one-field run's, bit for bit; r = nt identity probes against the sum over the stored (p, r) histories."""
+    is the one-field run's, bit for bit; r = nt identity probes against the sum over the stored (p, r) histories.
+    T > 1: time-blocked schedule (two half-slots per history slot, the flush roles see the r field as nx more rows)."""
     import oracle as orc
     from paper_2201_06914_b200 import Rtm, probes_dtt_host
     p = ri.random_tti(n=n, nb=12, nt=nt, r=r, seed=33)
     co = orc.coeffs(p)
-    one = run_gpu(p)
+    one = run_gpu(p, probe_block=T)
     offs = np.array([-3, 0, 2], np.int32)
     for Z in (p.Z, ri.identity_probes(p.nt)):
         rr = Z.shape[1]
         Zdd = probes_dtt_host(Z, p.dt)
-        m = Rtm.from_problem(p, r=rr, probe_fields=2)
+        m = Rtm.from_problem(p, r=rr, probe_fields=2, probe_block=T)
         m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
         m.set_probes(Zdd, Z)
         data = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz).cpu().numpy()
@@ -368,17 +370,25 @@ def test_tti_gradient_with_four_compressed_arrays(n, nt, r):
             assert rel(img, Iex) <= 1e-4, rel(img, Iex)
 
 
-def test_four_array_mode_is_for_fused_tti_probing_only():
-    from paper_2201_06914_b200 import Rtm, RTMError
+def test_four_array_mode_is_for_tti_and_does_not_depend_on_the_time_block():
+    from paper_2201_06914_b200 import Rtm, RTMError, probes_dtt_host
     pa = ri.random_acoustic(2, n=(30, 28), nb=4, nt=10, r=2)
     with pytest.raises(RTMError) as e:
         Rtm.from_problem(pa, probe_fields=2)
     assert e.value.code == -1
-    pt = ri.random_tti(n=(30, 28), nb=8, nt=10, r=2)
-    with pytest.raises(RTMError) as e:
-        Rtm.from_problem(pt, probe_fields=2, probe_block=8)
-    assert e.value.code == -1
-    Rtm.from_problem(pt, probe_fields=2, probe_block=1).close()
+    p = ri.random_tti(n=(75, 67), nb=12, nt=50, r=9, seed=33)
+    outs = []
+    for T in (1, 3, 8, 16):                      # reading C25: regrouped, not reordered -> bit-identical
+        m = Rtm.from_problem(p, probe_fields=2, probe_block=T)
+        m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        m.set_probes(probes_dtt_host(p.Z, p.dt), p.Z)
+        d = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+        img, _ = m.adjoint_image(p.rec_xyz, d, p.src_xyz)
+        outs.append([x.cpu().numpy() for x in (d, img, m.export_probes(0), m.export_probes(1))])
+        m.close()
+    for o in outs[1:]:
+        for x, y in zip(o, outs[0]):
+            assert np.array_equal(x, y)
 
 
 def test_qr_range_finder_probes():
