@@ -156,7 +156,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t o_rs = take((size_t)(nrows + 1) * 4);
     size_t o_en = take((size_t)c->max_pts * nc * sizeof(InjEntry));
     size_t o_si = take((size_t)c->max_pts * nc * 4), o_sw = take((size_t)c->max_pts * nc * 4);
-    size_t o_of = take(3 * 4096 * 4);
+    size_t o_of = take(5 * 4096 * 4);   // offsets / (ih, hx, hy) triples, then 512 run records of the tiled xy gather
     size_t o_dbg = take(1024 * 8 * 8);
     if (ctx) {
         char *b = ctx->ws;
@@ -244,7 +244,7 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
         CU(cudaMallocHost(&h.smp_w, (size_t)cfg->max_pts * nc * 4));
         CU(cudaEventCreateWithFlags(&h.done, cudaEventDisableTiming));
     }
-    CU(cudaMallocHost(&c->h_offs, 3 * 4096 * 4));
+    CU(cudaMallocHost(&c->h_offs, 5 * 4096 * 4));
     CU(cudaEventCreateWithFlags(&c->offs_done, cudaEventDisableTiming));
     *out = c;
     return RTM_OK;
@@ -852,8 +852,8 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
     for (int i = 1; i < nh && run; i++) run = h_offsets[i] == h_offsets[i - 1] + 1;
     if (run) {
         const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
-        if (nh <= 16) gather_tiled_kernel<16, false><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], 0, scale, d_gather);
-        else gather_tiled_kernel<GT_HP, false><<<grid, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], 0, scale, d_gather);
+        if (nh <= 16) gather_tiled_kernel<16, false><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], nullptr, 0, scale, d_gather);
+        else gather_tiled_kernel<GT_HP, false><<<grid, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], nullptr, 0, scale, d_gather);
     } else {
         const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
         gather_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->rp, nh, c->offs, scale, d_gather);
@@ -870,40 +870,45 @@ extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy,
         if (std::abs(h_offsets_xy[2 * i]) >= c->cfg.n[0] || std::abs(h_offsets_xy[2 * i + 1]) >= c->cfg.n[1]) return RTM_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Layout &L = c->L;
-    const long long N = (long long)L.nx * L.ny * L.nz;
     if (c->offs_pending) { CU(cudaEventSynchronize(c->offs_done)); c->offs_pending = false; }
-    // runs of consecutive hx at one hy (8..GT_HP long) take the register-tiled kernel, the rest the generic one
-    int nl = 0;
+    // runs of consecutive hx at one hy (8..GT_HP long) take the register-tiled kernel -- one launch for all runs of up
+    // to 16 offsets, one for the longer ones -- the rest go to the generic kernel as (ih, hx, hy) triples
+    int nl = 0, nrun[2] = {0, 0};
+    int *trip = c->h_offs, *run[2] = {c->h_offs + 3 * 4096, c->h_offs + 4 * 4096};
     for (int i = 0; i < nh;) {
         int j = i + 1;
         while (j < nh && j - i < GT_HP && h_offsets_xy[2 * j + 1] == h_offsets_xy[2 * i + 1] &&
                h_offsets_xy[2 * j] == h_offsets_xy[2 * (j - 1)] + 1)
             j++;
         if (j - i >= 8) {
-            const long long nblk = (((long long)L.ny * L.upz) / 32) * ((L.nx + GT_X - 1) / GT_X);   // x tiles fastest
-            if (nblk >= (1LL << 31)) return RTM_EINVAL;
-            const dim3 grid((unsigned)nblk, 1, 1);
-            if (j - i <= 16)
-                gather_tiled_kernel<16, true><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
-                                                                                   h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
-            else
-                gather_tiled_kernel<GT_HP, true><<<grid, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, j - i, h_offsets_xy[2 * i],
-                                                                                            h_offsets_xy[2 * i + 1], scale, d_gather + (long long)i * N);
-            c->launches++;
+            const int cls = j - i <= 16 ? 0 : 1;
+            int *rec = run[cls] + 4 * nrun[cls]++;
+            rec[0] = h_offsets_xy[2 * i]; rec[1] = h_offsets_xy[2 * i + 1]; rec[2] = j - i; rec[3] = i;
         } else {
             for (int m = i; m < j; m++) {
-                c->h_offs[3 * nl] = m;
-                c->h_offs[3 * nl + 1] = h_offsets_xy[2 * m];
-                c->h_offs[3 * nl + 2] = h_offsets_xy[2 * m + 1];
+                trip[3 * nl] = m;
+                trip[3 * nl + 1] = h_offsets_xy[2 * m];
+                trip[3 * nl + 2] = h_offsets_xy[2 * m + 1];
                 nl++;
             }
         }
         i = j;
     }
+    CU(cudaMemcpyAsync(c->offs, c->h_offs, (size_t)5 * 4096 * 4, cudaMemcpyHostToDevice, st));
+    CU(cudaEventRecord(c->offs_done, st));
+    c->offs_pending = true;
+    for (int cls = 0; cls < 2; cls++) {
+        if (!nrun[cls]) continue;
+        const long long nblk = (long long)L.ny * (L.upz / 32) * ((L.nx + GT_X - 1) / GT_X) * nrun[cls];
+        if (nblk >= (1LL << 31)) return RTM_EINVAL;
+        const int4 *d_runs = (const int4 *)(c->offs + (3 + cls) * 4096);
+        if (cls == 0)
+            gather_tiled_kernel<16, true><<<(unsigned)nblk, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, 0, 0, d_runs, nrun[cls], scale, d_gather);
+        else
+            gather_tiled_kernel<GT_HP, true><<<(unsigned)nblk, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, 0, 0, d_runs, nrun[cls], scale, d_gather);
+        c->launches++;
+    }
     if (nl) {
-        CU(cudaMemcpyAsync(c->offs, c->h_offs, (size_t)nl * 12, cudaMemcpyHostToDevice, st));
-        CU(cudaEventRecord(c->offs_done, st));
-        c->offs_pending = true;
         const long long tot = (long long)L.nx * L.ny * (L.upz / 4);
         gather_xy_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(L, c->Uz, c->Vz, c->rp, nl, c->offs, scale, d_gather);
         c->launches++;

@@ -94,7 +94,8 @@ def test_gather_xy_vector_offsets(n):
     p = ri.random_acoustic(3, n=n, nb=4, nt=120, r=5, seed=41, nsrc=1, nrec=6)
     box = [(hx, hy) for hy in range(-3, 4) for hx in range(-5, 6)]
     extra = [(0, 0), (n[0] - 1, 0), (0, n[1] - 1), (-2, 5), (3, -3), (n[0] // 2, -(n[1] // 2)), (1, 0), (2, 0)]
-    offs = np.array(box + extra, np.int32)
+    long_row = [(hx, 2) for hx in range(-10, 11)]              # 21 consecutive hx: the 48-offset instance
+    offs = np.array(box + extra + long_row, np.int32)
     hx_line = np.arange(-5, 6, dtype=np.int32)
     g, o, e = check_all(p, offsets=hx_line)
     gx = run_gpu(p, offsets_xy=offs)
@@ -116,6 +117,8 @@ def test_gather_xy_vector_offsets(n):
     # generic kernel (runs broken up by taking every other pair) == tiled kernel
     g2 = run_gpu(p, offsets_xy=offs[: len(box)][::2])
     assert np.array_equal(g2["gather_xy"], G[: len(box)][::2])
+    g3 = run_gpu(p, offsets_xy=np.array(long_row[::2], np.int32))
+    assert np.array_equal(g3["gather_xy"], G[len(box) + len(extra):][::2])
     # exact zeros wherever x + h or x - h leaves [0,nx) x [0,ny) (reading C28), for h and -h alike
     ix, iy = np.meshgrid(np.arange(n[0]), np.arange(n[1]), indexing="ij")
     for i, (hx, hy) in enumerate(offs):
