@@ -25,8 +25,12 @@
  * convergence in dt; TTI: H symmetric negative semi-definite, eps=delta=theta=0 => p == r ==
  * acoustic, theta -> theta+pi invariance; coefficient closed forms; two-field TTI probing (C29): central
  * differences of the misfit in K2 against sum_n (D p w_p + D r w_r) / (K2 h^2) from the histories.
- * PARITY UNPINNED (free choices no external fact fixes): the damping profile shape and strength,
- * the wavelet delay, and imaging the single TTI field (p+r)/2.
+ * Damped update (C7/C23): the centred scheme solved for the new level, stepped in numpy, to 1e-12 on the whole
+ * padded grid; in-layer attenuation exp(-int sigma/c) of the stated profile.  TTI kinematics (C10): homogeneous
+ * VTI is faster along x by sqrt(1 + 2 eps); with theta = +30 deg the fast direction is (cos th, -sin th).
+ * PARITY UNPINNED (free choices no external fact fixes; the implementation is pinned to its stated design, the
+ * design itself is a choice): the damping profile shape and strength, the wavelet delay, and imaging the single
+ * TTI field (p+r)/2.
  *
  * Grid layout: physical grid n = (nx,[ny],nz), absorbing layer nb on every side, padded grid
  * P = n + 2 nb; zeros outside P (reading C8).  z is the contiguous axis.  Internally every field
@@ -339,7 +343,7 @@ static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float
         t1 = malloc((size_t)g.NE * sizeof(double)); t2 = malloc((size_t)g.NE * sizeof(double));
         ma = calloc((size_t)g.NE, sizeof(double)); mb = calloc((size_t)g.NE, sizeof(double));
     }
-    if (PZ) memset(PZ, 0, sizeof(double) * (size_t)c->r * (size_t)g.N);
+    if (PZ) memset(PZ, 0, sizeof(double) * (size_t)np * (size_t)c->r * (size_t)g.N);
 
     for (int step = 0; step < c->nt; step++) {
         const int n = adjoint ? c->nt - 1 - step : step;
@@ -503,7 +507,7 @@ void orc_offset_gather(int nx, long nrest /* ny*nz */, int r, const double *Uz, 
 }
 
 /* Eq. 4 with a VECTOR horizontal offset h = (hx, hy) in grid points (
- * PAPER.md:L81 "generalize to 3D"; reading C26): 3D grids [nx][ny][nz],
+ * PAPER.md:L81 "generalize to 3D"; reading C28): 3D grids [nx][ny][nz],
  * G[ih][x] = scale * sum_k Uz[k][x + hx e_x + hy e_y] Vz[k][x - hx e_x - hy e_y];
  * zero when either shifted point leaves [0,nx) x [0,ny).  offs = [nh][2] = (hx, hy) pairs.         */
 void orc_offset_gather_xy(int nx, int ny, int nz, int r, const double *Uz, const double *Vz, int nh,

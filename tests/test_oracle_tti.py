@@ -177,3 +177,66 @@ def test_two_field_identity_probes_give_the_exact_sum_and_the_isotropic_limit():
     a1 = orc.adjoint(p, co, f2["samples"], Z=p.Z)
     I2, I1 = orc.image(f2["PZ"], a2["PZ"], 0.2), orc.image(f1["PZ"], a1["PZ"], 0.2)
     assert np.abs(I1).max() > 0 and np.abs(I2 - 2.0 * I1).max() <= 1e-12 * np.abs(I1).max()
+
+
+# ---- kinematics: which field carries eps-hat, and the sign of the tilt (reading C10) --------------------------------
+def _axis_velocities(theta_deg, eps=0.2, delta=0.1):
+    """Homogeneous TTI medium; velocity of the qP pulse along three directions from the peak-time difference of two
+    receivers 200 m apart on each ray: 'perp' = (cos th, -sin th) (perpendicular to the symmetry axis),
+    'axis' = (sin th, cos th) (along it), 'mirror' = (cos th, +sin th) (the perp direction of the medium tilted the
+    other way).  Cell-centred source and receivers (they neither excite nor record the Nyquist null space, C10)."""
+    import math
+    c, h, f0, n, nb = 2000.0, 10.0, 15.0, (121, 121), 20
+    th = math.radians(theta_deg)
+    src = np.array([[605.0, 605.0]])
+    dirs = {"perp": (math.cos(th), -math.sin(th)), "axis": (math.sin(th), math.cos(th)),
+            "mirror": (math.cos(th), math.sin(th))}
+    recs = []
+    for d in dirs.values():
+        for rho in (200.0, 400.0):
+            q = src[0] + rho * np.array(d)
+            recs.append((np.floor(q / h) + 0.5) * h)
+    recs = np.array(recs)
+    dt = 0.5 * ri.cfl_dt_tti(h, c, eps)
+    nt = int(0.45 / dt)
+    p = ri.homogeneous(2, n, h, c, f0, nt, 0.3, nb, src, recs)
+    p.dt, p.physics = dt, 1
+    t = np.arange(nt) * dt
+    a = (np.pi * f0 * (t - 1.0 / f0)) ** 2
+    p.wav = ((1.0 - 2.0 * a) * np.exp(-a)).astype(np.float32)[:, None].copy()
+    p.eps, p.delta, p.theta = (np.full(n, v, np.float32) for v in (eps, delta, th))
+    d = orc.forward(p, orc.coeffs(p))["samples"]
+
+    def peak_time(tr):
+        e = np.abs(tr)
+        i = int(np.argmax(e >= 0.5 * e.max()))                   # first arrival (the qP pulse), then its local peak
+        while i + 1 < len(e) and e[i + 1] >= e[i]:
+            i += 1
+        return (i + 0.5 * (e[i - 1] - e[i + 1]) / (e[i - 1] - 2.0 * e[i] + e[i + 1])) * dt
+
+    out = {}
+    for k, name in enumerate(dirs):
+        r0, r1 = recs[2 * k], recs[2 * k + 1]
+        out[name] = (np.linalg.norm(r1 - src[0]) - np.linalg.norm(r0 - src[0])) / (
+            peak_time(d[:, 2 * k + 1]) - peak_time(d[:, 2 * k])) / c
+    return out
+
+
+def test_vti_is_faster_along_x_by_sqrt_1_plus_2eps():
+    """theta = 0, eps = 0.2, delta = 0.1: the pulse travels at c sqrt(1 + 2 eps) along x and at c along z (the
+    symmetry axis).  Mutant it kills: H_perp / H_par swapped between the two fields (eps-hat moved from p to r),
+    which makes z the fast axis."""
+    v = _axis_velocities(0.0)
+    assert abs(v["perp"] / np.sqrt(1.4) - 1.0) <= 5e-3, v          # along x
+    assert abs(v["axis"] - 1.0) <= 5e-3, v                         # along z
+    assert abs(v["perp"] / v["axis"] / np.sqrt(1.4) - 1.0) <= 5e-3, v
+
+
+def test_tilt_sign_fast_direction_is_perpendicular_to_the_axis():
+    """theta = +30 deg tilts the symmetry axis n = (sin th, cos th) toward +x (reading C10): the fast direction is
+    (cos th, -sin th), perpendicular to n -- not its mirror image (cos th, +sin th), which is 60 deg away from it and
+    much slower.  Mutant it kills: sin(theta) taken with the opposite sign in tti_H (theta -> theta + pi cannot see it)."""
+    v = _axis_velocities(30.0)
+    assert abs(v["perp"] / np.sqrt(1.4) - 1.0) <= 5e-3, v
+    assert abs(v["axis"] - 1.0) <= 5e-3, v
+    assert v["mirror"] < 1.06 < v["perp"], v
