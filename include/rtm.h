@@ -12,8 +12,12 @@
  *   - pointer prefix d_ = device memory, h_ = host memory.  The caller owns every buffer,
  *     including the workspace; the library allocates and frees no device memory.
  *   - all device work is enqueued on the `cuda_stream` argument (a cudaStream_t passed as void*);
- *     no call synchronises the device.  Host tables (geometry) are built synchronously on the host
- *     and uploaded with cudaMemcpyAsync on the same stream.
+ *     no call synchronises the device.  Host tables (geometry, offsets) are built synchronously on the host
+ *     in pinned staging buffers of the context and uploaded with cudaMemcpyAsync on the same stream; a call
+ *     that needs a staging buffer whose previous upload (the previous call of the same kind) has not been
+ *     consumed yet waits on the host for that one copy (cudaEventSynchronize), never for kernels of its own.
+ *   - every call runs on the device that owns the workspace (taken from the pointer at rtm_create); the calling
+ *     thread's current device is restored on return.
  *   - grids: physical grid n = (nx,[ny],nz), z contiguous (C order [x][z] / [x][y][z]); absorbing
  *     layer of nb points on every side; padded grid P = n + 2 nb, Np = prod P, N = prod n.
  *     "canonical [Np]" / "[N]" arrays are dense C-order arrays without halo or pitch.
@@ -38,10 +42,11 @@ typedef struct {
     int ndim;       /* 2 | 3 */
     int n[3];       /* physical points: 2D (nx, nz, -) ; 3D (nx, ny, nz); z contiguous            */
     float h;        /* grid spacing [m], same on every axis                                       */
-    int nb;         /* absorbing-layer points on every side; must be a multiple of 4 (alignment)  */
+    int nb;         /* absorbing-layer points on every side, 0..1024 (any value: the internal z axis is
+                       shifted so that the physical grid stays float4-aligned)                      */
     int physics;    /* 0 isotropic acoustic ; 1 pseudo-acoustic TTI (ndim == 2 only)              */
     int nt;         /* time steps                                                                 */
-    double dt;      /* time step [s] (used by rtm_coeffs_host only)                               */
+    double dt;      /* time step [s] (used by rtm_coeffs_host only, which rejects dt <= 0 / non-finite) */
     int r;          /* number of probing vectors, 1..256 (Eq. 1)                    */
     int max_pts;    /* upper bound on nsrc and nrec of any later call (sizes geometry tables)     */
     int probe_block;/* T_b: 0|1 = probe fused into every time step (8 r bytes/point/step of Uz traffic);
@@ -124,6 +129,12 @@ int rtm_adjoint_image(rtm_ctx *ctx, int nrec, const float *h_rec_xyz, const floa
                       const float *h_src_xyz, float *d_qadj_out, float scale, int accumulate,
                       float *d_image, void *cuda_stream);
 
+/* The image alone, from the compressed wavefields the last forward and adjoint passes left in the context
+ * (Eq. 3):  image[x] (+)= scale * sum_k Uz[k][x] Vz[k][x].  Same kernel and same bits as the image
+ * rtm_adjoint_image writes; lets a caller re-image with another scale, or stack, without a new pass.
+ *   d_image canonical [N] (DEVICE).  Errors: RTM_EINVAL (NULL), RTM_ESTATE (no Uz/Vz yet).               */
+int rtm_image(rtm_ctx *ctx, float scale, int accumulate, float *d_image, void *cuda_stream);
+
 /* Horizontal subsurface-offset volumes (Eq. 4; reading C11):
  *   gather[ih][x] = scale * sum_k Uz[k][x + h e_x] Vz[k][x - h e_x],  h = h_offsets[ih] grid points
  *   along x, zero where x+h or x-h leaves [0,nx).  gather[h=0] == image (L52).
@@ -166,21 +177,28 @@ long long rtm_launch_count(const rtm_ctx *ctx);
  * on that pass's stream when option "time_steps" is 1.  Blocks the host until the pass has finished.
  * Negative if no timed pass has run.                                                               */
 float rtm_last_pass_ms(rtm_ctx *ctx, int which);
-/* Timing experiments (option "dbg" & 16): the first 8 phase time stamps (ns, %globaltimer) of each of the first
- * nblocks (<= 1024) blocks of the last step launch -> h_out [nblocks][8] (HOST).  Synchronises the device.  */
-int rtm_debug_stamps(rtm_ctx *ctx, unsigned long long *h_out, int nblocks);
-/* Tuning knobs and timing experiments; none of them changes what is computed:
+/* The same, averaged over the last `count` (1..64) timed passes of that kind (bench.py: the mean launch duration over
+ * the whole timed region, without a host synchronisation between shots).  Negative if fewer have run.      */
+float rtm_pass_ms_mean(rtm_ctx *ctx, int which, int count);
+/* Tuning knobs; none of them changes what is computed:
  *   "time_steps" 0|1  record CUDA events around the step launches of each pass (rtm_last_pass_ms);
  *   "pdl"        0|1  programmatic dependent launch between consecutive step kernels (default 1);
- *   "rx"         2|4|8|16|0  rows per thread of the 2D streaming kernel (0 = automatic; T > 1, 2D acoustic only);
- *   "dbg"        bit mask for timing experiments ONLY (results become wrong): 1 no flush role, 2 no stencil role,
- *                16 write phase time stamps (rtm_debug_stamps), 32 scalar arithmetic in the 3D streaming kernel
- *                (this one keeps the results bit-identical).
- * Errors: RTM_EINVAL (unknown name / value out of range).                                              */
+ *   "rx"         2|4|8|16|0  rows per thread of the 2D streaming kernel (0 = automatic; T > 1, 2D acoustic only).
+ * Errors: RTM_EINVAL (unknown name / value out of range).
+ * Timing experiments that break the results ("dbg" masks, per-block time stamps) exist only in a library built with
+ * -DRTM_DEBUG (see the end of this header); the product build has neither.                                */
 int rtm_set_option(rtm_ctx *ctx, const char *name, int value);
 
 const char *rtm_strerror(int code);
 const char *rtm_last_cuda_error(void);
+
+#ifdef RTM_DEBUG
+/* -DRTM_DEBUG builds only.  rtm_set_option(ctx, "dbg", mask): 1 no flush role, 2 no stencil role (RESULTS BECOME WRONG),
+ * 16 write phase time stamps, 32 scalar arithmetic in the 3D streaming kernel (T = 16; bit-identical results).
+ * rtm_debug_stamps: the first 8 phase time stamps (ns, %globaltimer) of each of the first nblocks (<= 1024) blocks of
+ * the last step launch -> h_out [nblocks][8] (HOST).  Synchronises the device.                               */
+int rtm_debug_stamps(rtm_ctx *ctx, unsigned long long *h_out, int nblocks);
+#endif
 
 #ifdef __cplusplus
 }

@@ -13,10 +13,10 @@ _LIBPATH = os.path.join(_HERE, "csrc", "librtm.so")
 _lib = None
 
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
-           "rtm_set_probes", "rtm_probes_dtt_host", "rtm_probes_qr_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_offset_gather",
+           "rtm_set_probes", "rtm_probes_dtt_host", "rtm_probes_qr_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_image", "rtm_offset_gather",
            "rtm_offset_gather_xy",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
-           "rtm_export_coeff", "rtm_debug_stamps", "rtm_last_pass_ms", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
+           "rtm_export_coeff", "rtm_last_pass_ms", "rtm_pass_ms_mean", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
 
 
 class RTMError(RuntimeError):
@@ -58,6 +58,7 @@ def load_library():
     lib.rtm_probes_qr_host.argtypes = [ip, ip, ip, vp, vp, vp]
     lib.rtm_forward_probe.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp]
     lib.rtm_adjoint_image.argtypes = [vp, ip, vp, vp, ip, vp, vp, fp, ip, vp, vp]
+    lib.rtm_image.argtypes = [vp, fp, ip, vp, vp]
     lib.rtm_offset_gather.argtypes = [vp, ip, vp, fp, vp, vp]
     lib.rtm_offset_gather_xy.argtypes = [vp, ip, vp, fp, vp, vp]
     lib.rtm_shot_staging_bytes.restype = C.c_size_t
@@ -66,11 +67,14 @@ def load_library():
     lib.rtm_export_probes.argtypes = [vp, ip, vp, vp]
     lib.rtm_set_snapshots.argtypes = [vp, ip, vp, vp]
     lib.rtm_export_coeff.argtypes = [vp, ip, vp, vp]
-    lib.rtm_debug_stamps.argtypes = [vp, vp, ip]
+    if hasattr(lib, "rtm_debug_stamps"):          # -DRTM_DEBUG builds only
+        lib.rtm_debug_stamps.argtypes = [vp, vp, ip]
     lib.rtm_launch_count.restype = C.c_longlong
     lib.rtm_launch_count.argtypes = [vp]
     lib.rtm_last_pass_ms.restype = C.c_float
     lib.rtm_last_pass_ms.argtypes = [vp, ip]
+    lib.rtm_pass_ms_mean.restype = C.c_float
+    lib.rtm_pass_ms_mean.argtypes = [vp, ip, ip]
     lib.rtm_set_option.argtypes = [vp, C.c_char_p, ip]
     lib.rtm_strerror.restype = C.c_char_p
     lib.rtm_strerror.argtypes = [ip]
@@ -278,6 +282,15 @@ class Rtm:
                                           self._ptr(q), sc, 1 if accumulate else 0, self._ptr(img), self._stream()))
         return img, q
 
+    def image(self, scale=None, out=None, accumulate=False):
+        """rtm_image: Eq. 3 from the Uz / Vz of the last forward and adjoint passes."""
+        t = self.torch
+        if out is None:
+            out = t.zeros(self.n, dtype=t.float32, device=self.device)
+        sc = 1.0 / self.r if scale is None else float(scale)
+        _check(self.lib.rtm_image(self.ctx, sc, 1 if accumulate else 0, self._ptr(out), self._stream()))
+        return out
+
     def offset_gather(self, offsets, scale=None, out=None):
         t = self.torch
         offs = np.ascontiguousarray(offsets, np.int32)
@@ -337,6 +350,8 @@ class Rtm:
         return out
 
     def debug_stamps(self, nblocks=1024):
+        if not hasattr(self.lib, "rtm_debug_stamps"):
+            raise RTMError(-1, "rtm_debug_stamps exists only in a library built with RTM_DEBUG=1")
         out = np.zeros((nblocks, 8), np.uint64)
         _check(self.lib.rtm_debug_stamps(self.ctx, _hp(out), int(nblocks)))
         return out
@@ -346,6 +361,9 @@ class Rtm:
 
     def last_pass_ms(self, which: int) -> float:
         return float(self.lib.rtm_last_pass_ms(self.ctx, int(which)))
+
+    def pass_ms_mean(self, which: int, count: int) -> float:
+        return float(self.lib.rtm_pass_ms_mean(self.ctx, int(which), int(count)))
 
     def set_option(self, name: str, value: int):
         _check(self.lib.rtm_set_option(self.ctx, name.encode(), int(value)))

@@ -25,7 +25,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+        dbg = ["-DRTM_DEBUG"] if os.environ.get("RTM_DEBUG") == "1" else []     # timing experiments (rtm.h, end)
+        cmd = [nvcc] + NVCC_FLAGS + dbg + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
         subprocess.check_call(cmd, cwd=CSRC)
         os.replace(tmp, LIB)
     return LIB

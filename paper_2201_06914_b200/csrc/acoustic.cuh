@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(256, ND == 2 ? 4 : 3) acoustic_step_kernel(con
     st4(a.n0 + off, unew);
 
     if (a.PZ != nullptr) {
-        const int ix = jx - L.nb, iy = jy - L.nby, iz = jz - L.nb;
+        const int ix = jx - L.nb, iy = jy - L.nby, iz = jz - L.nbz;
         if (ix >= 0 && ix < L.nx && iy >= 0 && iy < L.ny && iz >= 0 && iz < L.nz) {
             const long long o = ((long long)ix * L.ny + iy) * L.upz + iz;
             probe_quad<(ND == 2 ? 1 : 2)>(a.PZ + o, L.Nu, a.Zrow, a.r, unew);

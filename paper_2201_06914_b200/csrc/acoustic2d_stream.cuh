@@ -131,11 +131,11 @@ __global__ void __launch_bounds__(128, 4) acoustic2d_stream_kernel(const __grid_
             if (swt[c] != 0.0f) acc = fmaf(swt[c], u0[sidx[c]], acc);
         a.smp_out[task] = a.smp_scale * acc;
     }
-    if (active && (a.dbg & 3) != 2) {
+    if (active && !DBG_SKIP_STENCIL(a)) {
     const int sx = (int)L.sx;
     const int base = (int)L.org + jz;            // fsize < 2^31 (checked at create)
     const bool full = jz + 3 < L.Pz;
-    const int iz = jz - L.nb;
+    const int iz = jz - L.nbz;
     const bool zphys = iz >= 0 && iz < L.nz && a.hist != nullptr;
 
     float4 q[8 + RX];

@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     const float *pkk = K2 + oc;
     float *pd = d0 + oc;
     float *pn = n0 + oc;
-    const int iz = jz - L.nb, iy = jy - L.nby;
+    const int iz = jz - L.nbz, iy = jy - L.nby;
     const bool phys_yz = act && iz >= 0 && iz < L.nz && iy >= 0 && iy < L.ny && a.hist != nullptr;
     float *ph = a.hist + (((long long)(x0 - L.nb) * L.ny + iy) * L.upz + iz);   // dereferenced inside the physical grid only
     const long long hstep = (long long)L.ny * L.upz;

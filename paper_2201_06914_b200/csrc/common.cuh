@@ -12,12 +12,16 @@ namespace rtm {
 //  org + jx*sx + jy*sy + jz.  H = 4 (acoustic, order-8 star) or 8 (TTI, two chained order-8 first
 //  derivatives).  org, sx, sy are multiples of 4 floats so that z-quads (jz % 4 == 0) are float4-aligned.
 //  Compressed wavefields Uz/Vz: [k][ix][iy][iz] on the PHYSICAL grid only (reading C12), z pitch upz
-//  (multiple of 32), plane stride Nu.  nb % 4 == 0 keeps physical and padded quads aligned.
+//  (multiple of 32), plane stride Nu.  The internal z axis starts zs points before the padded grid so that the
+//  physical grid starts at a multiple of 4 (nbz): physical and padded quads are aligned for any nb.  Those zs
+//  points have K2 = 0 (and cos = sin = 0), so every field stays exactly zero there, like the halo.
 struct Layout {
     int nd;
     int nx, ny, nz;
-    int Px, Py, Pz;
-    int nb, nby;   // nby = nb in 3D, 0 in 2D (the dummy y axis has no layer)
+    int Px, Py, Pz;   // Pz is the INTERNAL z extent: zs alignment points (K2 = 0: they stay zero) + the padded grid
+    int Pzc, zs;      // canonical padded z extent nz + 2 nb; zs = (4 - nb % 4) % 4 makes nbz a multiple of 4
+    int nb, nby;      // nby = nb in 3D, 0 in 2D (the dummy y axis has no layer)
+    int nbz;          // internal z index of the first physical point = nb + zs
     int H, Hy;     // Hy = H in 3D, 0 in 2D
     int pz;
     long long sx, sy;
@@ -44,8 +48,10 @@ struct StepArgs {
     const float *dampx, *dampy, *dampz;
     const float *k1x, *k1y, *k1z;   // per-axis K1 tables: k1a[j] = (1 - damp_a[j]) / (1 + damp_a[j])
     int adjoint;
+#ifdef RTM_DEBUG
     int dbg;
     unsigned long long *dbg_ts;   // timing experiments (dbg & 16): per-phase %globaltimer stamps, [block][8]
+#endif
     // fused probe: PZ[k][x] += Zrow[k] * new[x]
     float *PZ;
     const float *Zrow;
@@ -157,11 +163,19 @@ __device__ __forceinline__ unsigned long long gtimer() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
+// Timing experiments exist in -DRTM_DEBUG builds only (paper_2201_06914_b200/build.py: RTM_DEBUG=1 in the environment);
+// the product library has neither the switches nor the stamps.
+#ifdef RTM_DEBUG
 #define DBG_STAMP(a, slot)                                                                  \
     do {                                                                                    \
         if (((a).dbg & 16) && threadIdx.x == 0 && threadIdx.y == 0 && blockIdx.x < 1024)    \
             (a).dbg_ts[blockIdx.x * 8 + (slot)] = gtimer();                                 \
     } while (0)
+#define DBG_SKIP_STENCIL(a) (((a).dbg & 3) == 2)
+#else
+#define DBG_STAMP(a, slot) do { } while (0)
+#define DBG_SKIP_STENCIL(a) false
+#endif
 
 // Flush role (time-blocked probing): PZ[k][x] += sum_{j<n} Z[n_j][k] hist[j][x] for this block's share of
 // the slice, one float2 of x per thread; T history values stay in registers while r planes stream through.

@@ -253,21 +253,21 @@ __global__ void __launch_bounds__(gt_threads(HP)) gather_tiled_kernel(Layout L, 
 // canonical [Np] -> internal haloed/pitched layout (halo untouched: it is zeroed once at create)
 __global__ void pack_field_kernel(Layout L, const float *__restrict__ src, float *__restrict__ dst) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long Np = (long long)L.Px * L.Py * L.Pz;
+    const long long Np = (long long)L.Px * L.Py * L.Pzc;
     if (t >= Np) return;
-    const int jz = (int)(t % L.Pz);
-    const long long q = t / L.Pz;
+    const int jz = (int)(t % L.Pzc);
+    const long long q = t / L.Pzc;
     const int jy = (int)(q % L.Py), jx = (int)(q / L.Py);
-    dst[L.org + jx * L.sx + jy * L.sy + jz] = src[t];
+    dst[L.org + jx * L.sx + jy * L.sy + jz + L.zs] = src[t];
 }
 __global__ void unpack_field_kernel(Layout L, const float *__restrict__ src, float *__restrict__ dst) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long Np = (long long)L.Px * L.Py * L.Pz;
+    const long long Np = (long long)L.Px * L.Py * L.Pzc;
     if (t >= Np) return;
-    const int jz = (int)(t % L.Pz);
-    const long long q = t / L.Pz;
+    const int jz = (int)(t % L.Pzc);
+    const long long q = t / L.Pzc;
     const int jy = (int)(q % L.Py), jx = (int)(q / L.Py);
-    dst[t] = src[L.org + jx * L.sx + jy * L.sy + jz];
+    dst[t] = src[L.org + jx * L.sx + jy * L.sy + jz + L.zs];
 }
 // internal probe planes -> canonical [r][N]
 // two != 0 (probe_fields = 2): r counts all 2 r_probes planes; canonical plane f r_probes + k = internal plane 2k + f

@@ -30,6 +30,17 @@ static thread_local char g_cuda_err[256] = "";
 
 static inline long long rup(long long v, long long m) { return (v + m - 1) / m * m; }
 
+// Every entry point runs on the device that owns the context's workspace, whatever device is current in the calling
+// thread; the previous device is restored on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 // pinned host staging for one set of geometry tables, guarded by an event so that a later call does
 // not overwrite it while an earlier upload is still in flight
 struct HostTables {
@@ -43,6 +54,7 @@ struct HostTables {
 
 struct rtm_ctx {
     rtm_config cfg;
+    int device;             // the device d_workspace lives on
     Layout L;
     char *ws;
     size_t ws_bytes;
@@ -73,11 +85,13 @@ struct rtm_ctx {
     float *snap_out;
     long long launches;
     int opt_time, opt_pdl, opt_dbg;
-    cudaEvent_t ev[2][2];
-    bool ev_valid[2];
+    static const int kEvRing = 64;
+    cudaEvent_t ev[2][kEvRing][2];   // [pass kind][ring slot][begin, end]: the last kEvRing timed passes of each kind
+    long long ev_count[2];           // timed passes recorded so far
 };
 
 static int pick_rx(rtm_ctx *c);
+static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace, size_t bytes);
 static size_t stream_smem(const rtm_ctx *c, int rx);
 static long long stream_blocks(const rtm_ctx *c, int rx);
 static int tm_of(int T);
@@ -87,8 +101,8 @@ static bool valid_cfg(const rtm_config *c) {
     if (c->ndim != 2 && c->ndim != 3) return false;
     for (int a = 0; a < c->ndim; a++)
         if (c->n[a] < 1 || c->n[a] > (1 << 14)) return false;
-    if (!(c->h > 0.f)) return false;
-    if (c->nb < 0 || c->nb % 4 != 0 || c->nb > 1024) return false;
+    if (!(c->h > 0.f) || !std::isfinite(c->h)) return false;
+    if (c->nb < 0 || c->nb > 1024) return false;
     if (c->physics != 0 && c->physics != 1) return false;
     if (c->physics == 1 && c->ndim != 2) return false;
     if (c->nt < 1 || c->r < 1 || c->r > 256 || c->max_pts < 1) return false;
@@ -114,7 +128,10 @@ static void make_layout(const rtm_config *c, Layout *L) {
     L->Hy = c->ndim == 3 ? L->H : 0;
     L->Px = L->nx + 2 * c->nb;
     L->Py = L->ny + 2 * L->nby;
-    L->Pz = L->nz + 2 * c->nb;
+    L->Pzc = L->nz + 2 * c->nb;
+    L->zs = (4 - c->nb % 4) % 4;          // alignment points in front of the padded grid (K2 = 0 there)
+    L->nbz = c->nb + L->zs;
+    L->Pz = L->Pzc + L->zs;
     L->pz = (int)rup(L->Pz + 2 * L->H + 4, 32);
     L->sy = L->pz;
     L->sx = (long long)(L->Py + 2 * L->Hy) * L->pz;
@@ -204,21 +221,26 @@ extern "C" size_t rtm_workspace_bytes(const rtm_config *cfg) {
     return carve(cfg, L, nullptr);
 }
 
-static bool is_device_ptr(const void *p) {
-    cudaPointerAttributes at;
-    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
-    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
-}
-
 extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes, rtm_ctx **out) {
     if (!out) return RTM_EINVAL;
     *out = nullptr;
     size_t need = rtm_workspace_bytes(cfg);
     if (need == 0 || !d_workspace || ((uintptr_t)d_workspace & 255)) return RTM_EINVAL;
     if (bytes < need) return RTM_ENOMEM;
-    if (!is_device_ptr(d_workspace)) return RTM_EINVAL;
+    cudaPointerAttributes pat;
+    if (cudaPointerGetAttributes(&pat, d_workspace) != cudaSuccess) { cudaGetLastError(); return RTM_EINVAL; }
+    if (pat.type != cudaMemoryTypeDevice && pat.type != cudaMemoryTypeManaged) return RTM_EINVAL;
     rtm_ctx *c = new (std::nothrow) rtm_ctx();
     if (!c) return RTM_ENOMEM;
+    c->device = pat.device;
+    DeviceGuard guard(c->device);   // events, pinned tables and the occupancy query belong to the workspace's device
+    int rc = create_on_device(c, cfg, d_workspace, bytes);
+    if (rc) { rtm_destroy(c); return rc; }   // rtm_ctx() value-initialises its pointers: a partial context is safe to destroy
+    *out = c;
+    return RTM_OK;
+}
+
+static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace, size_t bytes) {
     c->cfg = *cfg;
     make_layout(cfg, &c->L);
     c->ws = (char *)d_workspace;
@@ -231,9 +253,10 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     c->opt_pdl = 1;
     c->opt_dbg = 0;
     c->rx = (cfg->ndim == 2 && cfg->physics == 0 && c->T > 0) ? pick_rx(c) : 0;
-    c->ev_valid[0] = c->ev_valid[1] = false;
+    c->ev_count[0] = c->ev_count[1] = 0;
     for (int i = 0; i < 2; i++)
-        for (int j = 0; j < 2; j++) CU(cudaEventCreate(&c->ev[i][j]));
+        for (int s = 0; s < rtm_ctx::kEvRing; s++)
+            for (int j = 0; j < 2; j++) CU(cudaEventCreate(&c->ev[i][s][j]));
     c->offs_pending = false;
     const int nc = 1 << cfg->ndim;
     for (int t = 0; t < 2; t++) {
@@ -246,12 +269,12 @@ extern "C" int rtm_create(const rtm_config *cfg, void *d_workspace, size_t bytes
     }
     CU(cudaMallocHost(&c->h_offs, 5 * 4096 * 4));
     CU(cudaEventCreateWithFlags(&c->offs_done, cudaEventDisableTiming));
-    *out = c;
     return RTM_OK;
 }
 
 extern "C" void rtm_destroy(rtm_ctx *c) {
     if (!c) return;
+    DeviceGuard guard(c->device);
     for (int t = 0; t < 2; t++) {
         HostTables &h = c->ht[t];
         if (h.done) { cudaEventSynchronize(h.done); cudaEventDestroy(h.done); }
@@ -260,7 +283,8 @@ extern "C" void rtm_destroy(rtm_ctx *c) {
     if (c->offs_done) { cudaEventSynchronize(c->offs_done); cudaEventDestroy(c->offs_done); }
     cudaFreeHost(c->h_offs);
     for (int i = 0; i < 2; i++)
-        for (int j = 0; j < 2; j++) if (c->ev[i][j]) cudaEventDestroy(c->ev[i][j]);
+        for (int s = 0; s < rtm_ctx::kEvRing; s++)
+            for (int j = 0; j < 2; j++) if (c->ev[i][s][j]) cudaEventDestroy(c->ev[i][s][j]);
     delete c;
 }
 
@@ -269,6 +293,7 @@ extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const f
                                const float *h_theta, float *h_K2, float *h_epsh, float *h_delh, float *h_cos,
                                float *h_sin, float *h_damp1d) {
     if (!valid_cfg(cfg) || !h_vp || !h_K2 || !h_damp1d) return RTM_EINVAL;
+    if (!(cfg->dt > 0.0) || !std::isfinite(cfg->dt)) return RTM_EINVAL;   // K2 and the damping tables would be 0 or NaN
     const bool tti = cfg->physics == 1;
     if (tti && (!h_eps || !h_delta || !h_theta || !h_epsh || !h_delh || !h_cos || !h_sin)) return RTM_EINVAL;
     Layout L;
@@ -280,7 +305,7 @@ extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const f
     for (long long i = 0; i < N; i++) vmax = std::max(vmax, (double)h_vp[i]);
     const double sigma_max = nb > 0 ? vmax * std::log(1000.0) / ((double)nb * h) : 0.0;
     // per-axis profiles sigma_a(i) dt; the dummy y axis of a 2D grid contributes nothing
-    const int P[3] = {L.Px, L.Py, L.Pz};
+    const int P[3] = {L.Px, L.Py, L.Pzc};
     const int lay[3] = {nb, L.nby, nb};
     std::vector<double> prof[3];
     float *tab = h_damp1d;
@@ -299,12 +324,12 @@ extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const f
     const int nn[3] = {L.nx, L.ny, L.nz};
     for (int jx = 0; jx < L.Px; jx++)
         for (int jy = 0; jy < L.Py; jy++)
-            for (int jz = 0; jz < L.Pz; jz++) {
+            for (int jz = 0; jz < L.Pzc; jz++) {
                 const int ix = std::min(std::max(jx - lay[0], 0), nn[0] - 1);
                 const int iy = std::min(std::max(jy - lay[1], 0), nn[1] - 1);
                 const int iz = std::min(std::max(jz - lay[2], 0), nn[2] - 1);
                 const long long s = ((long long)ix * L.ny + iy) * L.nz + iz;
-                const long long d = ((long long)jx * L.Py + jy) * L.Pz + jz;
+                const long long d = ((long long)jx * L.Py + jy) * L.Pzc + jz;
                 const double c = h_vp[s];
                 const double sdt = prof[0][jx] + prof[1][jy] + prof[2][jz];
                 h_K2[d] = (float)(c * c * dt * dt / (h * h * (1.0 + sdt)));
@@ -375,7 +400,7 @@ extern "C" int rtm_probes_qr_host(int nt, int nrec, int r, const float *h_D, con
 }
 
 static int launch_pack(rtm_ctx *c, const float *src, float *dst, cudaStream_t st) {
-    const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pz;
+    const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pzc;
     pack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, st>>>(c->L, src, dst);
     c->launches++;
     CU(cudaGetLastError());
@@ -385,6 +410,7 @@ static int launch_pack(rtm_ctx *c, const float *src, float *dst, cudaStream_t st
 extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh, const float *d_delh,
                              const float *d_cos, const float *d_sin, const float *h_damp1d, void *stream) {
     if (!c || !d_K2 || !h_damp1d) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     const bool tti = c->cfg.physics == 1;
     if (tti && (!d_epsh || !d_delh || !d_cos || !d_sin)) return RTM_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -407,7 +433,7 @@ extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh,
         CU(cudaMemcpyAsync(c->dampy, t, (size_t)L.Py * 4, cudaMemcpyHostToDevice, st));
         t += L.Py;
     }
-    CU(cudaMemcpyAsync(c->dampz, t, (size_t)L.Pz * 4, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(c->dampz + L.zs, t, (size_t)L.Pzc * 4, cudaMemcpyHostToDevice, st));   // the zs alignment points keep 0
     // per-axis K1 tables, computed on the device with the same division the kernels use at layer corners
     k1_table_kernel<<<(L.Px + 32 + 255) / 256, 256, 0, st>>>(c->dampx, c->k1x, L.Px + 32);
     k1_table_kernel<<<(L.Py + 8 + 255) / 256, 256, 0, st>>>(c->dampy, c->k1y, L.Py + 8);
@@ -421,6 +447,7 @@ extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh,
 
 extern "C" int rtm_set_probes(rtm_ctx *c, const float *d_Zf, const float *d_Za, void *stream) {
     if (!c || !d_Zf || !d_Za) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     const long long tot = (long long)c->cfg.nt * c->zr;
     pack_probes_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(c->cfg.nt, c->cfg.r, c->zr, d_Zf, c->Zf);
@@ -461,7 +488,7 @@ static int corners_of(const rtm_config &cfg, const Layout &L, const float *xyz, 
                 w *= bz ? frac[2] : 1.0 - frac[2];
                 co.jx = base[0] + bx + L.nb;
                 co.jy = base[1] + by + L.nby;
-                co.jz = base[2] + bz + L.nb;
+                co.jz = base[2] + bz + L.nbz;
                 co.w = (float)w;
             }
     return cnt;
@@ -577,9 +604,8 @@ static step_fn stream2d_fn(int rx) {
 // Rows per thread of the 2D streaming kernel: the smallest RX in {2,4,8,16} whose launch (stencil + flush blocks) fits
 // in two waves of resident blocks; larger problems use 4.
 static int pick_rx(rtm_ctx *c) {
-    int dev = 0, nsm = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    int nsm = 148;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->device);
     const int tm = tm_of(c->T);
     // flush-role blocks that share every launch: one float4 of the physical grid per thread, 1/T of it per step
     const long long quads = (long long)c->L.nx * c->L.ny * (c->L.upz / (c->T <= 16 ? 4 : 2));
@@ -612,13 +638,15 @@ static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, 
     lc.gridDim = dim3(nblocks, 1, 1); lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
     lc.attrs = at; lc.numAttrs = 1;
     if (smem > 48 * 1024) {   // opt in to large dynamic shared memory, once per kernel and size
-        static thread_local std::vector<std::pair<const void *, size_t>> done;
+        // (the attribute is per device: the cache is keyed by it)
+        struct Done { int dev; const void *fp; size_t smem; };
+        static thread_local std::vector<Done> done;
         const void *fp = (const void *)kernel;
         bool ok = false;
-        for (auto &d : done) ok = ok || (d.first == fp && d.second >= smem);
+        for (auto &d : done) ok = ok || (d.dev == c->device && d.fp == fp && d.smem >= smem);
         if (!ok) {
             CU(cudaFuncSetAttribute(fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            done.push_back({fp, smem});
+            done.push_back({c->device, fp, smem});
         }
     }
     CU(cudaLaunchKernelEx(&lc, kernel, a));
@@ -654,8 +682,12 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
             case 0: return launch_ex(c, acoustic_step_kernel<3>, a, nb, block, 0, st);
             case 4: return launch_ex(c, acoustic3d_stream_kernel<4, true>, a, nb, block, smem, st);
             case 8: return launch_ex(c, acoustic3d_stream_kernel<8, true>, a, nb, block, smem, st);
+#ifdef RTM_DEBUG
             case 16: return (c->opt_dbg & 32) ? launch_ex(c, acoustic3d_stream_kernel<16, false>, a, nb, block, smem, st)
                                               : launch_ex(c, acoustic3d_stream_kernel<16, true>, a, nb, block, smem, st);
+#else
+            case 16: return launch_ex(c, acoustic3d_stream_kernel<16, true>, a, nb, block, smem, st);
+#endif
             default: return launch_ex(c, acoustic3d_stream_kernel<32, true>, a, nb, block, smem, st);
         }
     }
@@ -723,9 +755,10 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     const bool deferred = want_smp && (long long)g.nsmp <= nblocks * bthreads;
     const unsigned smp_blocks = (unsigned)((g.nsmp + 255) / 256);
 
-    if (c->opt_time) CU(cudaEventRecord(c->ev[adjoint][0], st));
+    const int evs = (int)(c->ev_count[adjoint] % rtm_ctx::kEvRing);
+    if (c->opt_time) CU(cudaEventRecord(c->ev[adjoint][evs][0], st));
     int cur = 0;
-    const long long Np = (long long)L.Px * L.Py * L.Pz;
+    const long long Np = (long long)L.Px * L.Py * L.Pzc;
     for (int step = 0; step < nt; step++) {
         const int n = adjoint ? nt - 1 - step : step;
         const int nprev = adjoint ? n + 1 : n - 1;
@@ -759,9 +792,11 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
                 }
             }
         }
+#ifdef RTM_DEBUG
         if ((c->opt_dbg & 3) == 1) a.fl_blocks = 0;
         a.dbg = c->opt_dbg;
         a.dbg_ts = c->dbg_ts;
+#endif
         { int rc_ = launch_step(c, a, grid, block, smem, st); if (rc_) return rc_; }
         cur ^= 1;
         if (T && step == nt - 1) {   // the last time block has no following steps to hide behind
@@ -769,7 +804,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
             const int nfirst = adjoint ? nt - 1 - fb * T : fb * T;
             launch_flush(c, c->hist + (size_t)(fb & 1) * T * c->pNu, lenf, Z + (size_t)nfirst * c->zr, a.fl_zstep, PZ, st);
         }
-        if (c->opt_time && step == nt - 1) { CU(cudaEventRecord(c->ev[adjoint][1], st)); c->ev_valid[adjoint] = true; }
+        if (c->opt_time && step == nt - 1) { CU(cudaEventRecord(c->ev[adjoint][evs][1], st)); c->ev_count[adjoint]++; }
         if (want_smp && (!deferred || step == nt - 1)) {
             StepArgs s = a;   // sample the field just computed
             s.u0 = c->fld[0][cur]; s.u1 = c->fld[1][cur];
@@ -794,6 +829,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
 extern "C" int rtm_forward_probe(rtm_ctx *c, int nsrc, const float *h_src_xyz, const float *d_wav, int nrec,
                                  const float *h_rec_xyz, float *d_data_out, void *stream) {
     if (!c || nsrc < 1 || !h_src_xyz || !d_wav || nrec < 0 || (nrec > 0 && !h_rec_xyz)) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     if (nsrc > c->cfg.max_pts || nrec > c->cfg.max_pts) return RTM_EINVAL;
     if (!c->have_model || !c->have_probes) return RTM_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -821,6 +857,7 @@ extern "C" int rtm_adjoint_image(rtm_ctx *c, int nrec, const float *h_rec_xyz, c
                                  const float *h_src_xyz, float *d_qadj_out, float scale, int accumulate,
                                  float *d_image, void *stream) {
     if (!c || nrec < 1 || !h_rec_xyz || !d_data_in || nsrc < 0 || (nsrc > 0 && !h_src_xyz)) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     if (nsrc > c->cfg.max_pts || nrec > c->cfg.max_pts) return RTM_EINVAL;
     if (!c->have_model || !c->have_probes) return RTM_ESTATE;
     if (d_image && !c->have_U) return RTM_ESTATE;   // adjoint before forward
@@ -836,8 +873,16 @@ extern "C" int rtm_adjoint_image(rtm_ctx *c, int nrec, const float *h_rec_xyz, c
     return RTM_OK;
 }
 
+extern "C" int rtm_image(rtm_ctx *c, float scale, int accumulate, float *d_image, void *stream) {
+    if (!c || !d_image) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
+    if (!c->have_U || !c->have_V) return RTM_ESTATE;
+    return launch_image(c, scale, accumulate, d_image, (cudaStream_t)stream);
+}
+
 extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float scale, float *d_gather, void *stream) {
     if (!c || nh < 1 || nh > 4096 || !h_offsets || !d_gather) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     if (!c->have_U || !c->have_V) return RTM_ESTATE;
     for (int i = 0; i < nh; i++)
         if (std::abs(h_offsets[i]) >= c->cfg.n[0]) return RTM_EINVAL;
@@ -865,6 +910,7 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
 
 extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy, float scale, float *d_gather, void *stream) {
     if (!c || nh < 1 || nh > 4096 || !h_offsets_xy || !d_gather || c->cfg.ndim != 3) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     if (!c->have_U || !c->have_V) return RTM_ESTATE;
     for (int i = 0; i < nh; i++)
         if (std::abs(h_offsets_xy[2 * i]) >= c->cfg.n[0] || std::abs(h_offsets_xy[2 * i + 1]) >= c->cfg.n[1]) return RTM_EINVAL;
@@ -935,6 +981,18 @@ extern "C" int rtm_shot_host(rtm_ctx *c, int nsrc, const float *h_src_xyz, const
                              float *h_image, int nh, const int *h_offsets, float *h_gather, void *d_staging,
                              size_t staging_bytes, void *stream) {
     if (!c || !h_wav || !h_data_in || !d_staging) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
+    // everything a later stage would reject is rejected before any work is enqueued
+    if (nsrc < 1 || nrec < 1 || !h_src_xyz || !h_rec_xyz || nsrc > c->cfg.max_pts || nrec > c->cfg.max_pts) return RTM_EINVAL;
+    if (nh < 0 || nh > 4096 || (nh > 0 && h_gather && !h_offsets)) return RTM_EINVAL;
+    for (int i = 0; i < nh && h_gather; i++)
+        if (std::abs(h_offsets[i]) >= c->cfg.n[0]) return RTM_EINVAL;
+    if (!c->have_model || !c->have_probes) return RTM_ESTATE;
+    {
+        Corner co[8];
+        for (int s = 0; s < nsrc; s++) if (corners_of(c->cfg, c->L, h_src_xyz + (size_t)s * c->cfg.ndim, co) < 0) return RTM_EINVAL;
+        for (int s = 0; s < nrec; s++) if (corners_of(c->cfg, c->L, h_rec_xyz + (size_t)s * c->cfg.ndim, co) < 0) return RTM_EINVAL;
+    }
     size_t need = rtm_shot_staging_bytes(&c->cfg, nsrc, nrec, nh);
     if (need == 0 || ((uintptr_t)d_staging & 255)) return RTM_EINVAL;
     if (staging_bytes < need) return RTM_ENOMEM;
@@ -966,6 +1024,7 @@ extern "C" int rtm_shot_host(rtm_ctx *c, int nsrc, const float *h_src_xyz, const
 // ---- test hooks ----------------------------------------------------------------------------------
 extern "C" int rtm_export_probes(rtm_ctx *c, int which, float *d_out, void *stream) {
     if (!c || !d_out || (which != 0 && which != 1)) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     if (which == 0 ? !c->have_U : !c->have_V) return RTM_ESTATE;
     const Layout &L = c->L;
     const long long tot = (long long)L.nx * L.ny * L.nz * c->rp;
@@ -984,31 +1043,42 @@ extern "C" int rtm_set_snapshots(rtm_ctx *c, int nsnap, const int *h_steps, floa
 
 extern "C" int rtm_export_coeff(rtm_ctx *c, int which, float *d_out, void *stream) {
     if (!c || !d_out || which < 0 || which > 4) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     if (!c->have_model) return RTM_ESTATE;
     const float *src[5] = {c->K2, c->epsh, c->delh, c->cs, c->sn};
     if (!src[which]) return RTM_EINVAL;
-    const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pz;
+    const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pzc;
     unpack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c->L, src[which], d_out);
     c->launches++;
     CU(cudaGetLastError());
     return RTM_OK;
 }
 
-extern "C" float rtm_last_pass_ms(rtm_ctx *c, int which) {
-    if (!c || (which != 0 && which != 1) || !c->ev_valid[which]) return -1.0f;
-    if (cudaEventSynchronize(c->ev[which][1]) != cudaSuccess) return -1.0f;
-    float ms = -1.0f;
-    if (cudaEventElapsedTime(&ms, c->ev[which][0], c->ev[which][1]) != cudaSuccess) return -1.0f;
-    return ms;
+extern "C" float rtm_pass_ms_mean(rtm_ctx *c, int which, int count) {
+    if (!c || (which != 0 && which != 1) || count < 1 || count > rtm_ctx::kEvRing || c->ev_count[which] < count) return -1.0f;
+    DeviceGuard guard(c->device);
+    double sum = 0.0;
+    for (int i = 1; i <= count; i++) {
+        const int s = (int)((c->ev_count[which] - i) % rtm_ctx::kEvRing);
+        if (cudaEventSynchronize(c->ev[which][s][1]) != cudaSuccess) return -1.0f;
+        float ms = -1.0f;
+        if (cudaEventElapsedTime(&ms, c->ev[which][s][0], c->ev[which][s][1]) != cudaSuccess) return -1.0f;
+        sum += ms;
+    }
+    return (float)(sum / count);
 }
+extern "C" float rtm_last_pass_ms(rtm_ctx *c, int which) { return rtm_pass_ms_mean(c, which, 1); }
 
+#ifdef RTM_DEBUG
 // timing experiments: copy the per-block phase stamps of the last launch (dbg & 16) to the host; synchronises
 extern "C" int rtm_debug_stamps(rtm_ctx *c, unsigned long long *h_out, int nblocks) {
     if (!c || !h_out || nblocks < 1 || nblocks > 1024) return RTM_EINVAL;
+    DeviceGuard guard(c->device);
     CU(cudaDeviceSynchronize());
     CU(cudaMemcpy(h_out, c->dbg_ts, (size_t)nblocks * 8 * 8, cudaMemcpyDeviceToHost));
     return RTM_OK;
 }
+#endif
 
 extern "C" long long rtm_launch_count(const rtm_ctx *c) { return c ? c->launches : 0; }
 
@@ -1016,9 +1086,13 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!c || !name) return RTM_EINVAL;
     if (!strcmp(name, "time_steps")) { c->opt_time = value; return RTM_OK; }
     if (!strcmp(name, "pdl")) { c->opt_pdl = value; return RTM_OK; }
+#ifdef RTM_DEBUG
     if (!strcmp(name, "dbg")) { c->opt_dbg = value; return RTM_OK; }   // timing experiments only: 1 = no flush role, 2 = no stencil
+#endif
     if (!strcmp(name, "rx")) {   // rows per thread of the 2D streaming kernel (2|4|8|16); 0 = automatic
         if (!c->rx) return RTM_EINVAL;
+        if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16) return RTM_EINVAL;   // the kernel's instances
+        DeviceGuard guard(c->device);
         c->rx = value > 0 ? value : pick_rx(c);
         return RTM_OK;
     }

@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const St
     st4(a.n1 + off, make_float4(rn[0], rn[1], rn[2], rn[3]));
 
     if (TM > 0 ? (a.hist != nullptr) : (a.PZ != nullptr)) {
-        const int ix = jx - L.nb, iz = jz - L.nb;
+        const int ix = jx - L.nb, iz = jz - L.nbz;
         if (ix >= 0 && ix < L.nx && iz >= 0 && iz < L.nz) {
             const long long o = (long long)ix * L.upz + iz;
             const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);

@@ -23,6 +23,8 @@ def test_library_exports_every_declared_symbol():
     lib = B.load_library()
     hdr = open(os.path.join(ROOT, "include", "rtm.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    hdr = re.sub(r"#ifdef RTM_DEBUG.*?#endif", "", hdr, flags=re.S)      # timing experiments: -DRTM_DEBUG builds only
+    assert not hasattr(lib, "rtm_debug_stamps")                          # the product library has no debug switches
     declared = sorted(set(re.findall(r"\b(rtm_[a-z_]+)\s*\(", hdr)))
     assert len(declared) >= 15
     for name in declared:
@@ -91,6 +93,22 @@ def test_host_coefficients_match_oracle_bitwise():
         if p.physics == 1:
             for a, b in ((eh, co.epsh), (dh, co.delh), (cs, co.cosT), (sn, co.sinT)):
                 assert np.array_equal(a, b)
+
+
+def test_coeffs_host_rejects_bad_time_step_and_spacing():
+    """dt <= 0 or non-finite would give K2 = 0 / NaN tables with RTM_OK: rejected instead."""
+    _build()
+    from paper_2201_06914_b200 import RTMError
+    from paper_2201_06914_b200 import binding as B
+    p = ri.random_acoustic(2, n=(12, 10), nb=4, nt=5)
+    for dt in (0.0, -1e-3, float("nan"), float("inf")):
+        with pytest.raises(RTMError) as e:
+            B.coeffs_host(B.make_config(p.ndim, p.n, p.h, p.nb, 0, p.nt, dt, p.r, 8), p.vp)
+        assert e.value.code == -1
+    for h in (float("inf"), float("nan"), 0.0):
+        assert B.workspace_bytes(B.make_config(p.ndim, p.n, h, p.nb, 0, p.nt, p.dt, p.r, 8)) == 0
+    for nb in (0, 3, 5, 6, 7):                                  # any layer thickness is a valid config (no nb % 4 rule)
+        assert B.workspace_bytes(B.make_config(p.ndim, p.n, p.h, nb, 0, p.nt, p.dt, p.r, 8)) > 0
 
 
 def test_qr_probes_host_match_oracle():

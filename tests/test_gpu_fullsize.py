@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import rtm_inputs as ri
-from gpu_util import TOL_FIELD, TOL_IMAGE, rel, run_gpu, run_oracle
+from gpu_util import TOL_FIELD, TOL_IMAGE, elem_ok, rel, run_gpu, run_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -33,6 +33,18 @@ def test_c1_full_shot_against_oracle():
     for k in ("Uz", "Vz", "image", "gather"):
         assert errs[k] <= TOL_IMAGE, (k, errs)
     assert np.array_equal(g["gather"][20], g["image"])          # h = 0 is the zero-offset image, bit for bit
+    ref = {"data": f["samples"], "qadj": a["samples"], "Uz": f["PZ"], "Vz": a["PZ"], "image": img, "gather": gat}
+    for k, o in ref.items():
+        elem_ok(g[k], o, TOL_FIELD if k in ("data", "qadj") else TOL_IMAGE, "c1 T=32 " + k)
+    # the per-step-fused schedule (probe_block = 0: acoustic_step_kernel<2>, north_star's literal design) on the same
+    # whole shot against the same oracle results
+    g0 = run_gpu(p, din=din, offsets=p.offsets, probe_block=0)
+    errs0 = {k: rel(g0[k], o) for k, o in ref.items()}
+    print("c1 full, per-step fused", {k: "%.2e" % v for k, v in errs0.items()})
+    for k, o in ref.items():
+        tol = TOL_FIELD if k in ("data", "qadj") else TOL_IMAGE
+        assert errs0[k] <= tol, (k, errs0)
+        elem_ok(g0[k], o, tol, "c1 T=0 " + k)
 
 
 def test_c2_full_grid_short_record():
@@ -79,3 +91,30 @@ def test_c4_full_grid_properties():
     # sampled outputs against the oracle: the forward pass of the full grid for the same 24 steps (about half a minute of CPU)
     f = orc.forward(p, orc.coeffs(p))
     assert rel(d16, f["samples"]) <= TOL_FIELD, rel(d16, f["samples"])
+
+
+def test_3d_streaming_kernel_many_tiles_against_oracle():
+    """A c4-shaped volume large enough for 8 y-tiles (8 rows each), 3 z-tiles (128 points, the last one ragged) and
+    7 x-chunks (32 planes, the last one ragged) of acoustic3d_stream_kernel, with sources and receivers scattered
+    over the whole volume so that every tile carries signal: data, adjoint traces, Uz, Vz, image and a 9-offset
+    gather against the oracle, element by element (the largest 3D case checked against the
+    oracle was 104 x 96 x 88)."""
+    p = ri.random_acoustic(3, n=(160, 24, 260), nb=20, nt=48, r=16, seed=41, nsrc=12, nrec=400)
+    assert p.P == (200, 64, 300)
+    offs = np.arange(-4, 5, dtype=np.int32)
+    for T in (32, 16):
+        g = run_gpu(p, offsets=offs, probe_block=T)
+        if T == 32:
+            o = run_oracle(p, g["din"], offsets=offs)
+        errs = {k: rel(g[k], o[k]) for k in ("data", "qadj", "Uz", "Vz", "image", "gather")}
+        print("3D many tiles T=%d" % T, {k: "%.2e" % v for k, v in errs.items()})
+        for k in errs:
+            tol = TOL_FIELD if k in ("data", "qadj") else TOL_IMAGE
+            assert errs[k] <= tol, (k, errs)
+            elem_ok(g[k], o[k], tol, "T=%d %s" % (T, k))
+        # every tile of the volume took part: the image is non-zero in all 8 octants
+        img = g["image"].reshape(p.n)
+        for sx in (slice(0, 80), slice(80, 160)):
+            for sy in (slice(0, 12), slice(12, 24)):
+                for sz in (slice(0, 130), slice(130, 260)):
+                    assert np.abs(img[sx, sy, sz]).max() > 0

@@ -48,6 +48,19 @@ def test_tti_random_offgrid(n, nb, r):
     check_all(p, snap_steps=[10, 40, 79], offsets=np.array([-1, 0, 4], np.int32))
 
 
+@pytest.mark.parametrize("nb", [1, 2, 3, 5, 6, 7])
+def test_layer_thickness_need_not_be_a_multiple_of_4(nb):
+    """Any nb: the internal z axis starts (4 - nb % 4) % 4 points before the padded grid (K2 = 0 there) so that the
+    physical grid stays float4-aligned; results must still be the oracle's (which has no such points)."""
+    p = ri.random_acoustic(2, n=(70, 61), nb=nb, nt=60, r=6, seed=31, nsrc=2, nrec=5)
+    check_all(p, snap_steps=[30, 59], offsets=np.array([-2, 0, 1], np.int32))
+    check_all(p, snap_steps=[59], offsets=np.arange(-4, 5, dtype=np.int32), probe_block=5)
+    p3 = ri.random_acoustic(3, n=(21, 18, 37), nb=nb, nt=40, r=5, seed=32)
+    check_all(p3, snap_steps=[39], probe_block=4 if nb % 2 else 0)
+    q = ri.random_tti(n=(75, 67), nb=nb + 4, nt=50, r=5, seed=33)
+    check_all(q, snap_steps=[49], offsets=np.array([-1, 0, 3], np.int32), probe_block=8 if nb % 2 else 0)
+
+
 def test_c1_cropped():
     p = ri.make_c3(n=(256, 200), nt=600, r=32, nb=80)
     import oracle as orc
