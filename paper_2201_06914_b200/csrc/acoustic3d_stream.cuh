@@ -115,62 +115,81 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     float *__restrict__ n0 = a.n0;
     float *d0 = a.d0;
 
-    // what this thread may request: its centre quad (also when it only feeds a neighbour's halo) ...
-    const bool ld_c = jz + 8 <= L.pz && jy < L.Py + 4;
-    // ... one quad of the y halo (rows -4..-1 and 8..11 of the tile) ...
-    const int hrow = ty < 4 ? ty : ty + S3_TY;                 // smem row of the halo quad
-    const int jyh = (int)by * S3_TY + hrow - 4;
-    const bool ld_h = jz + 8 <= L.pz && jyh < L.Py + 4;
-    // ... and, for the first / last lane of a row, one quad of the z halo
-    const bool zl = tx == 0, zr_ = tx == 31;
-    const bool ld_z = (zl || (zr_ && jz + 12 <= L.pz)) && jy < L.Py + 4;
-
     const long long sx = L.sx;
     const long long oc = L.org + (long long)x0 * sx + (long long)jy * L.sy + jz;
     const float *pc = u0 + oc;                                  // centre quad, plane x0
-    const float *phh = u0 + L.org + (long long)x0 * sx + (long long)jyh * L.sy + jz;
-    const float *pkk = K2 + oc;
-    float *pd = d0 + oc;
-    float *pn = n0 + oc;
     const int iz = jz - L.nbz, iy = jy - L.nby;
     const bool phys_yz = act && iz >= 0 && iz < L.nz && iy >= 0 && iy < L.ny && a.hist != nullptr;
-    float *ph = a.hist + (((long long)(x0 - L.nb) * L.ny + iy) * L.upz + iz);   // dereferenced inside the physical grid only
     const long long hstep = (long long)L.ny * L.upz;
 
     float *Ub = dyn_smem;                                        // [S3_NU][S3_ROWS][S3_PITCH]
     float *Kb = Ub + S3_NU * S3_TILE;                            // [S3_NK][S3_TY][S3_TZ]
     float *Db = Kb + S3_NK * S3_CT;
     const int o_c = (ty + 4) * S3_PITCH + 4 + tx * 4;            // this thread's centre slot inside a u tile
-    const int o_h = hrow * S3_PITCH + 4 + tx * 4;                // its y-halo slot
     const int o_k = tid * 4;
     const int last_pl = min(nplanes + 3, L.Px + 3 - x0);         // last plane (relative to x0) any thread needs
 
-    // request the haloed u tile of plane `pl` (relative to x0); planes nobody needs are skipped
-    auto request_u = [&](int pl) {
-        if (pl > last_pl) return;
-        float *t = Ub + (pl & (S3_NU - 1)) * S3_TILE;
-        const long long o = (long long)pl * sx;
-        cp_async16(t + o_c, ld_c ? pc + o : u0, ld_c);
-        cp_async16(t + o_h, ld_h ? phh + o : u0, ld_h);
-        if (zl) cp_async16(t + o_c - 4, ld_z ? pc + o - 4 : u0, ld_z);
-        if (zr_) cp_async16(t + o_c + 4, ld_z ? pc + o + 4 : u0, ld_z);
+    // Request descriptors, all loop-invariant: what this thread copies for every plane is fixed up to the plane
+    // stride, so the source pointers are RUNNING pointers (one 64-bit add per plane each) and the shared-memory
+    // destinations are a slot base plus constants -- no per-plane index / bound / 64-bit multiply arithmetic (the
+    // round-1 kernel spent ~70 of its ~450 instructions per plane on that).  A thread that has nothing to fetch for
+    // one of its three u quads keeps a valid pointer with stride 0 and a source size of 0 (zero fill).
+    //   quad 1: its centre quad (also when it only feeds a neighbour's halo);
+    //   quad 2: one quad of the y halo (rows -4..-1 and 8..11 of the tile);
+    //   quad 3: for the first / last lane of a row, one quad of the z halo.
+    const int hrow = ty < 4 ? ty : ty + S3_TY;                 // smem row of the halo quad
+    const int jyh = (int)by * S3_TY + hrow - 4;
+    const bool ld_c = jz + 8 <= L.pz && jy < L.Py + 4;
+    const bool ld_h = jz + 8 <= L.pz && jyh < L.Py + 4;
+    const bool zl = tx == 0, zr_ = tx == 31;
+    const bool ld_z = (zl || (zr_ && jz + 12 <= L.pz)) && jy < L.Py + 4;
+    const float *rq_c = ld_c ? pc : u0;
+    const float *rq_h = ld_h ? u0 + L.org + (long long)x0 * sx + (long long)jyh * L.sy + jz : u0;
+    const float *rq_z = ld_z ? pc + (zl ? -4 : 4) : u0;
+    const long long st_c = ld_c ? sx : 0, st_h = ld_h ? sx : 0, st_z = ld_z ? sx : 0;
+    const int o_h = hrow * S3_PITCH + 4 + tx * 4;                // its y-halo slot
+    const int o_z = o_c + (zl ? -4 : 4);                         // its z-halo slot (first / last lane only)
+    const bool has_z = zl || zr_;
+    const float *rq_k = K2 + oc;
+    const float *rq_d = d0 + oc;
+    int rq_us = 0, rq_ks = 0;                                    // ring slots of the next u / (K2, du) request
+    int pl_u = 0, pl_k = 0;                                      // planes they belong to (relative to x0)
+
+    // request the haloed u tile of the next plane; planes nobody needs are skipped
+    auto request_u = [&]() {
+        if (pl_u <= last_pl) {
+            float *t = Ub + rq_us * S3_TILE;
+            cp_async16(t + o_c, rq_c, ld_c);
+            cp_async16(t + o_h, rq_h, ld_h);
+            if (has_z) cp_async16(t + o_z, rq_z, ld_z);
+        }
+        rq_c += st_c; rq_h += st_h; rq_z += st_z;
+        rq_us = (rq_us + 1) & (S3_NU - 1);
+        pl_u++;
     };
-    auto request_kd = [&](int pl) {
-        if (pl >= nplanes || !act) return;
-        const long long o = (long long)pl * sx;
-        cp_async16(Kb + (pl & (S3_NK - 1)) * S3_CT + o_k, pkk + o, true);
-        cp_async16(Db + (pl & (S3_NK - 1)) * S3_CT + o_k, pd + o, true);
+    auto request_kd = [&]() {
+        if (pl_k < nplanes && act) {
+            cp_async16(Kb + rq_ks * S3_CT + o_k, rq_k, true);
+            cp_async16(Db + rq_ks * S3_CT + o_k, rq_d, true);
+        }
+        rq_k += sx; rq_d += sx;
+        rq_ks = (rq_ks + 1) & (S3_NK - 1);
+        pl_k++;
     };
     // pipeline prologue: S3_D groups; group g of iteration p carries u plane p+4+D and K2/du plane p+D
-    request_u(0); request_u(1); request_u(2); request_u(3); request_u(4);
-    request_kd(0);
+    request_u(); request_u(); request_u(); request_u(); request_u();
+    request_kd();
     cp_async_commit();
 #pragma unroll
     for (int g = 1; g < S3_D; g++) {
-        request_u(4 + g);
-        request_kd(g);
+        request_u();
+        request_kd();
         cp_async_commit();
     }
+    // running output pointers (this thread's quad of plane x0 + p)
+    float *pd = d0 + oc;
+    float *pn = n0 + oc;
+    float *ph = a.hist + (((long long)(x0 - L.nb) * L.ny + iy) * L.upz + iz);   // dereferenced inside the physical grid only
 
     const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
     float4 q[9];   // planes p-4 .. p+4 of this thread's quad; q[8] is filled from the ring at the top of iteration p
@@ -184,8 +203,8 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     for (int p = 0; p < nplanes; p++) {
         cp_async_wait<S3_D - 1>();   // this thread's requests of groups <= p - D ... p + 0 - D have landed
         __syncthreads();             // everybody's have; and nobody reads the slots the next request overwrites
-        request_u(p + 4 + S3_D);
-        request_kd(p + S3_D);
+        request_u();
+        request_kd();
         cp_async_commit();
 
         const float *U0 = Ub + (p & (S3_NU - 1)) * S3_TILE + o_c;            // current plane, centre slot
@@ -259,10 +278,11 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
                 if (jz + 2 >= L.Pz) { dn.z = 0.f; un.z = 0.f; }
                 dn.w = 0.f; un.w = 0.f;
             }
-            st4(pd + (long long)p * sx, dn);
-            st4(pn + (long long)p * sx, un);
-            if (phys_yz && (unsigned)(jx - L.nb) < (unsigned)L.nx) stcs4(ph + (long long)p * hstep, un);
+            st4(pd, dn);
+            st4(pn, un);
+            if (phys_yz && (unsigned)(jx - L.nb) < (unsigned)L.nx) stcs4(ph, un);
         }
+        pd += sx; pn += sx; ph += hstep;
         // slide the x queue by one plane
 #pragma unroll
         for (int i = 0; i < 8; i++) q[i] = q[i + 1];
