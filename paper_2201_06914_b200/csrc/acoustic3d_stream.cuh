@@ -1,20 +1,21 @@
-// acoustic3d_stream.cuh -- 3D isotropic acoustic time step (a1) for time-blocked probing: 2.5D blocking with an
-// asynchronous shared-memory pipeline.
+// acoustic3d_stream.cuh -- 3D isotropic acoustic time step (a1) for time-blocked probing: 2.5D blocking fed by the
+// tensor memory accelerator.
 //
 // Block = 256 threads = a (y, z) tile of 8 x 128 points, one z-quad (float4) per thread, streaming along the
 // slow axis x over a chunk of S3_XCH planes.
-//   - every global read goes through cp.async (LDGSTS, 16 B, zero-fill outside the allocated halo) into rings in
-//     shared memory, S3_D planes ahead of its use: the haloed u tile of plane p+4+D and the K2 / du tiles of
-//     plane p+D are requested while plane p is computed.  The bytes in flight live in shared memory, not in
-//     registers (a register-prefetch version of this kernel kept 64 B per thread in flight and stalled at 59 %
-//     of the DRAM roofline: memory-level parallelism, not instruction issue, was the limit);
+//   - every tile comes through TMA (cp.async.bulk.tensor, SASS UTMALDG): ONE thread asks for the haloed 16 x 136 box
+//     of u of plane p+4+D and the 8 x 128 boxes of K2 and du of plane p+D while plane p is computed; the bytes land
+//     in rings in shared memory and are counted on an mbarrier per group.  No thread spends instructions on
+//     addresses, bounds or zero fill (the round-1 cp.async version spent ~70 of its ~450 instructions per plane and
+//     quad on exactly that, plus the registers that forced the compiler to recompute loop invariants); boxes that
+//     stick out of the allocation are zero-filled by the copy engine, which is the boundary condition (C8);
 //   - x neighbours: a 9-deep register queue per thread that slides one plane per iteration and is fed from the
 //     ring when a plane arrives;
 //   - y and z neighbours: read from the ring slot of the current plane (halo of 4 in y and z);
-//   - one __syncthreads per plane: it publishes the arrived plane and frees the slot the next request overwrites.
-// Per plane and quad: 5 LDGSTS + 12 LDS.128 + 3 STG.128, arithmetic in packed fp32x2 (FADD2 / FFMA2).  DRAM
-// traffic stays at the algorithmic 20 B/point (u, du read; u', du' written; K2): the x re-reads of neighbouring
-// chunks and the y/z halos hit L2.
+//   - one __syncthreads per plane: it frees the slots the next request overwrites.
+// Per plane and quad: 13 LDS.128 + 3 STG.128, arithmetic in packed fp32x2 (FADD2 / FFMA2).  DRAM traffic stays at the
+// algorithmic 20 B/point (u, du read; u', du' written; K2): the x re-reads of neighbouring chunks and the y/z halos
+// hit L2.
 //
 // Fused as in the 2D kernel: damping through per-axis K1 tables, source injection (a3; the block's injection
 // amounts are looked up by all 256 threads in parallel before griddepcontrol.wait), deferred receiver sampling
@@ -34,8 +35,10 @@ constexpr int S3_NK = 4;                // K2 / du ring slots = S3_D + 1
 constexpr int S3_TILE = S3_ROWS * S3_PITCH;      // floats per haloed u tile
 constexpr int S3_CT = S3_TY * S3_TZ;             // floats per K2 / du tile
 constexpr int S3_INJCAP = 512;          // injection amounts (float4) a block can stage
-constexpr int S3_SMEM = (S3_NU * S3_TILE + 2 * S3_NK * S3_CT) * 4 + S3_INJCAP * 16;
-static_assert(S3_NU == 5 + S3_D && S3_NK == S3_D + 1, "ring sizes follow the prefetch distance");
+constexpr int S3_NB = 4;                // mbarriers: groups p .. p+D are in flight
+constexpr int S3_SMEM = (S3_NU * S3_TILE + 2 * S3_NK * S3_CT) * 4 + S3_INJCAP * 16 + S3_NB * 8;
+static_assert(S3_NU == 5 + S3_D && S3_NK == S3_D + 1 && S3_NB == S3_D + 1, "ring sizes follow the prefetch distance");
+static_assert((S3_TILE * 4) % 128 == 0 && (S3_CT * 4) % 128 == 0, "TMA destinations stay 128-byte aligned");
 
 // sum of the injection entries of padded row `row` that fall into the z-quad starting at jz (a3)
 __device__ __forceinline__ float4 inject_lookup(const StepArgs &a, long long row, int jz) {
@@ -56,7 +59,7 @@ __device__ __forceinline__ float4 inject_lookup(const StepArgs &a, long long row
 
 template <int TM, bool PK>
 __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_constant__ StepArgs a) {
-    extern __shared__ __align__(16) float dyn_smem[];
+    extern __shared__ __align__(128) float dyn_smem[];
     const Layout &L = a.L;
     const int tid = threadIdx.x;
     if (blockIdx.x < (unsigned)a.fl_blocks) {
@@ -74,6 +77,11 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     const bool act = jz < L.Pz && jy < L.Py;
 
     float4 *injs = reinterpret_cast<float4 *>(dyn_smem + S3_NU * S3_TILE + 2 * S3_NK * S3_CT);   // [S3_INJCAP], behind the rings
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(injs + S3_INJCAP);          // [S3_NB] mbarriers
+    if (tid == 0) {
+        for (int i = 0; i < S3_NB; i++) mbar_init(bars + i, 1);   // one arrival (thread 0's expect_tx) + the bytes
+        mbar_fence_init();
+    }
 
     // ---- prologue on static data (before the grid dependency is resolved) ----------------------------------
     // injection: all (plane, row, z-quad) triples of this block's tile that intersect the bounding box of the
@@ -106,6 +114,7 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     }
     const bool zdamp = (dzv[0] != 0.f) | (dzv[1] != 0.f) | (dzv[2] != 0.f) | (dzv[3] != 0.f);
 
+    __syncthreads();   // the mbarriers are initialised (and the staged injection amounts visible) before anybody waits
     pdl_wait();   // from here on the previous step's fields are complete and visible
     pdl_launch_dependents();   // only now: lets the next step's flush role run without a wait (see flush_role)
     sample_points(a, lin_block, 256, tid);
@@ -127,65 +136,27 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     float *Db = Kb + S3_NK * S3_CT;
     const int o_c = (ty + 4) * S3_PITCH + 4 + tx * 4;            // this thread's centre slot inside a u tile
     const int o_k = tid * 4;
-    const int last_pl = min(nplanes + 3, L.Px + 3 - x0);         // last plane (relative to x0) any thread needs
+    const bool ld_c = jz + 8 <= L.pz && jy < L.Py + 4;           // its centre quad exists in the allocation
 
-    // Request descriptors, all loop-invariant: what this thread copies for every plane is fixed up to the plane
-    // stride, so the source pointers are RUNNING pointers (one 64-bit add per plane each) and the shared-memory
-    // destinations are a slot base plus constants -- no per-plane index / bound / 64-bit multiply arithmetic (the
-    // round-1 kernel spent ~70 of its ~450 instructions per plane on that).  A thread that has nothing to fetch for
-    // one of its three u quads keeps a valid pointer with stride 0 and a source size of 0 (zero fill).
-    //   quad 1: its centre quad (also when it only feeds a neighbour's halo);
-    //   quad 2: one quad of the y halo (rows -4..-1 and 8..11 of the tile);
-    //   quad 3: for the first / last lane of a row, one quad of the z halo.
-    const int hrow = ty < 4 ? ty : ty + S3_TY;                 // smem row of the halo quad
-    const int jyh = (int)by * S3_TY + hrow - 4;
-    const bool ld_c = jz + 8 <= L.pz && jy < L.Py + 4;
-    const bool ld_h = jz + 8 <= L.pz && jyh < L.Py + 4;
-    const bool zl = tx == 0, zr_ = tx == 31;
-    const bool ld_z = (zl || (zr_ && jz + 12 <= L.pz)) && jy < L.Py + 4;
-    const float *rq_c = ld_c ? pc : u0;
-    const float *rq_h = ld_h ? u0 + L.org + (long long)x0 * sx + (long long)jyh * L.sy + jz : u0;
-    const float *rq_z = ld_z ? pc + (zl ? -4 : 4) : u0;
-    const long long st_c = ld_c ? sx : 0, st_h = ld_h ? sx : 0, st_z = ld_z ? sx : 0;
-    const int o_h = hrow * S3_PITCH + 4 + tx * 4;                // its y-halo slot
-    const int o_z = o_c + (zl ? -4 : 4);                         // its z-halo slot (first / last lane only)
-    const bool has_z = zl || zr_;
-    const float *rq_k = K2 + oc;
-    const float *rq_d = d0 + oc;
-    int rq_us = 0, rq_ks = 0;                                    // ring slots of the next u / (K2, du) request
-    int pl_u = 0, pl_k = 0;                                      // planes they belong to (relative to x0)
+    // Group g = the haloed u tile of plane g+4 (group 0: planes 0..4) and the K2 / du tiles of plane g, relative to
+    // x0; planes 0 .. nplanes+3 of u are needed, so a group is needed iff g < nplanes.  Tensor coordinates are
+    // (z, y, x) counted from the first allocated float of a field: padded index + halo (4 on every axis here).
+    const char *tmaps = (const char *)a.tmaps;
+    const void *tm_u = tmaps + 128 * a.tm_u, *tm_k = tmaps + 256, *tm_d = tmaps + 384;
+    const int cz = (int)bz * S3_TZ, cy = (int)by * S3_TY, cx = x0 + 4;      // the box of u starts 4 before the tile
+    auto issue = [&](int g) {                                    // thread 0 only
+        if (g >= nplanes) return;
+        unsigned long long *bar = bars + (g & (S3_NB - 1));
+        mbar_arrive_expect_tx(bar, (unsigned)((g == 0 ? 5 : 1) * S3_TILE * 4 + 2 * S3_CT * 4));
+        if (g == 0)
+            for (int pl = 0; pl < 4; pl++) tma_load_3d(Ub + pl * S3_TILE, tm_u, cz, cy, cx + pl, bar);
+        tma_load_3d(Ub + ((g + 4) & (S3_NU - 1)) * S3_TILE, tm_u, cz, cy, cx + g + 4, bar);
+        tma_load_3d(Kb + (g & (S3_NK - 1)) * S3_CT, tm_k, cz + 4, cy + 4, cx + g, bar);
+        tma_load_3d(Db + (g & (S3_NK - 1)) * S3_CT, tm_d, cz + 4, cy + 4, cx + g, bar);
+    };
+    if (tid == 0)
+        for (int g = 0; g < S3_D; g++) issue(g);
 
-    // request the haloed u tile of the next plane; planes nobody needs are skipped
-    auto request_u = [&]() {
-        if (pl_u <= last_pl) {
-            float *t = Ub + rq_us * S3_TILE;
-            cp_async16(t + o_c, rq_c, ld_c);
-            cp_async16(t + o_h, rq_h, ld_h);
-            if (has_z) cp_async16(t + o_z, rq_z, ld_z);
-        }
-        rq_c += st_c; rq_h += st_h; rq_z += st_z;
-        rq_us = (rq_us + 1) & (S3_NU - 1);
-        pl_u++;
-    };
-    auto request_kd = [&]() {
-        if (pl_k < nplanes && act) {
-            cp_async16(Kb + rq_ks * S3_CT + o_k, rq_k, true);
-            cp_async16(Db + rq_ks * S3_CT + o_k, rq_d, true);
-        }
-        rq_k += sx; rq_d += sx;
-        rq_ks = (rq_ks + 1) & (S3_NK - 1);
-        pl_k++;
-    };
-    // pipeline prologue: S3_D groups; group g of iteration p carries u plane p+4+D and K2/du plane p+D
-    request_u(); request_u(); request_u(); request_u(); request_u();
-    request_kd();
-    cp_async_commit();
-#pragma unroll
-    for (int g = 1; g < S3_D; g++) {
-        request_u();
-        request_kd();
-        cp_async_commit();
-    }
     // running output pointers (this thread's quad of plane x0 + p)
     float *pd = d0 + oc;
     float *pn = n0 + oc;
@@ -201,11 +172,9 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     float sxn = a.dampx[x0], k1xn = a.k1x[x0];   // x damping of the next plane, fetched one iteration ahead
 #pragma unroll 1
     for (int p = 0; p < nplanes; p++) {
-        cp_async_wait<S3_D - 1>();   // this thread's requests of groups <= p - D ... p + 0 - D have landed
-        __syncthreads();             // everybody's have; and nobody reads the slots the next request overwrites
-        request_u();
-        request_kd();
-        cp_async_commit();
+        __syncthreads();             // nobody reads the slots (and the mbarrier) the next group overwrites any more
+        if (tid == 0) issue(p + S3_D);
+        mbar_wait(bars + (p & (S3_NB - 1)), (unsigned)(p / S3_NB) & 1u);   // group p has landed: u plane p+4, K2 / du plane p
 
         const float *U0 = Ub + (p & (S3_NU - 1)) * S3_TILE + o_c;            // current plane, centre slot
         q[8] = ld4(Ub + ((p + 4) & (S3_NU - 1)) * S3_TILE + o_c);
@@ -287,7 +256,6 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
 #pragma unroll
         for (int i = 0; i < 8; i++) q[i] = q[i + 1];
     }
-    cp_async_wait<0>();
 }
 
 }  // namespace rtm

@@ -52,6 +52,9 @@ struct StepArgs {
     int dbg;
     unsigned long long *dbg_ts;   // timing experiments (dbg & 16): per-phase %globaltimer stamps, [block][8]
 #endif
+    // 3D streaming kernel: four CUtensorMaps (128 B each) in device memory: u ping, u pong, K2, du (rtm.cu: make_tmaps)
+    const void *tmaps;
+    int tm_u;               // which of the two u maps describes u0 in this launch
     // fused probe: PZ[k][x] += Zrow[k] * new[x]
     float *PZ;
     const float *Zrow;
@@ -149,6 +152,35 @@ __device__ __forceinline__ void cp_async16(float *dst_smem, const float *src, bo
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// ---- TMA (cp.async.bulk.tensor) + mbarrier: one elected thread asks the copy engine for a whole box of a tensor
+// described by a CUtensorMap; the bytes land in shared memory and are counted on an mbarrier the consumers wait on.
+// (SASS: UTMALDG / SYNCS.)  Out-of-bounds parts of a box are filled with zeros.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// one arrival that also announces `bytes` of copy-engine traffic for the current phase
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// Wait for the phase with the given parity.  try_wait sleeps in hardware for a bounded time; the retry count is bounded
+// too, so a descriptor or byte-count bug ends in a trap (a CUDA error on the host), never in a hung GPU.
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    const unsigned a = smem_u32(bar);
+    unsigned done = 0;
+    for (int it = 0; it < (1 << 22); it++) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+        if (done) return;
+    }
+    __trap();
+}
+__device__ __forceinline__ void tma_load_3d(void *dst_smem, const void *tmap, int c0, int c1, int c2, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst_smem)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
 
 // Programmatic dependent launch: let the next step's grid become resident while this one drains, and
 // wait for the previous grid (and its memory) before touching anything it wrote.

@@ -7,6 +7,8 @@
 #include <new>
 #include <vector>
 
+#include <cuda.h>   // CUtensorMap (types only: the encoder is fetched through cudaGetDriverEntryPoint, no -lcuda)
+
 #include "../../include/rtm.h"
 #include "acoustic.cuh"
 #include "acoustic2d_stream.cuh"
@@ -75,6 +77,7 @@ struct rtm_ctx {
     float *smp_w;
     int *offs;
     unsigned long long *dbg_ts;
+    void *tmaps;            // 4 CUtensorMaps of the 3D streaming kernel (u ping, u pong, K2, du), device memory
     long long nrows;
     bool have_model, have_probes, have_U, have_V;
     HostTables ht[2];       // [0] forward call, [1] adjoint call
@@ -91,6 +94,7 @@ struct rtm_ctx {
 };
 
 static int pick_rx(rtm_ctx *c);
+static int make_tmaps(rtm_ctx *c);
 static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace, size_t bytes);
 static size_t stream_smem(const rtm_ctx *c, int rx);
 static long long stream_blocks(const rtm_ctx *c, int rx);
@@ -175,6 +179,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t o_si = take((size_t)c->max_pts * nc * 4), o_sw = take((size_t)c->max_pts * nc * 4);
     size_t o_of = take(5 * 4096 * 4);   // offsets / (ih, hx, hy) triples, then 512 run records of the tiled xy gather
     size_t o_dbg = take(1024 * 8 * 8);
+    size_t o_tm = take(4 * 128);
     if (ctx) {
         char *b = ctx->ws;
         ctx->nf = nf;
@@ -208,6 +213,7 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->smp_w = (float *)(b + o_sw);
         ctx->offs = (int *)(b + o_of);
         ctx->dbg_ts = (unsigned long long *)(b + o_dbg);
+        ctx->tmaps = b + o_tm;
         ctx->nrows = nrows;
     }
     return off;
@@ -269,6 +275,7 @@ static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace
     }
     CU(cudaMallocHost(&c->h_offs, 5 * 4096 * 4));
     CU(cudaEventCreateWithFlags(&c->offs_done, cudaEventDisableTiming));
+    if (cfg->ndim == 3 && cfg->physics == 0 && c->T > 0) return make_tmaps(c);
     return RTM_OK;
 }
 
@@ -552,6 +559,42 @@ static int build_geometry(rtm_ctx *c, int slot, int ninj, const float *inj_xyz, 
     return RTM_OK;
 }
 
+// ---- tensor maps of the 3D streaming kernel (TMA, acoustic3d_stream.cuh) ---------------------------------------
+// A field is a dense [Px + 2H][Py + 2H][pz] array of floats (halo included); the kernel asks for boxes by (z, y, x)
+// counted from the first float.  u ping / pong: haloed boxes 136 x 16 x 1; K2, du: 128 x 8 x 1.  Whatever part of a
+// box lies outside the array is filled with zeros by the copy engine.
+static int make_tmaps(rtm_ctx *c) {
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled is not available in this driver");
+        return RTM_ECUDA;
+    }
+    const Layout &L = c->L;
+    const cuuint64_t dims[3] = {(cuuint64_t)L.pz, (cuuint64_t)(L.Py + 2 * L.Hy), (cuuint64_t)(L.Px + 2 * L.H)};
+    const cuuint64_t strides[2] = {(cuuint64_t)L.sy * 4, (cuuint64_t)L.sx * 4};
+    const cuuint32_t ones[3] = {1, 1, 1};
+    const cuuint32_t box_u[3] = {(cuuint32_t)S3_PITCH, (cuuint32_t)S3_ROWS, 1}, box_k[3] = {(cuuint32_t)S3_TZ, (cuuint32_t)S3_TY, 1};
+    alignas(64) CUtensorMap maps[4];
+    static_assert(sizeof(CUtensorMap) == 128, "the kernel addresses the maps at multiples of 128 bytes");
+    void *base[4] = {c->fld[0][0], c->fld[0][1], c->K2, c->fld[0][2]};
+    for (int i = 0; i < 4; i++) {
+        CUresult r = ((encode_fn)fn)(&maps[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base[i], dims, strides, i < 2 ? box_u : box_k,
+                                     ones, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled failed with CUresult %d (map %d)", (int)r, i);
+            return RTM_ECUDA;
+        }
+    }
+    CU(cudaMemcpy(c->tmaps, maps, sizeof maps, cudaMemcpyHostToDevice));
+    return RTM_OK;
+}
+
 // ---- one propagation pass (a1-a6) ---------------------------------------------------------------
 static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
     const Layout &L = c->L;
@@ -765,6 +808,8 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
         a.u0 = c->fld[0][cur]; a.n0 = c->fld[0][cur ^ 1]; a.d0 = c->fld[0][2];
         a.u1 = c->fld[1][cur]; a.n1 = c->fld[1][cur ^ 1]; a.d1 = c->fld[1][2];
         a.Zrow = Z + (size_t)n * c->zr;
+        a.tmaps = c->tmaps;
+        a.tm_u = cur;
         a.inj_val = d_inj_val + (size_t)n * g.ninj;
         a.smp_out = (deferred && step > 0) ? d_smp_out + (size_t)nprev * g.nsmp : nullptr;
         a.fl_blocks = 0;
