@@ -183,7 +183,13 @@ float rtm_pass_ms_mean(rtm_ctx *ctx, int which, int count);
 /* Tuning knobs; none of them changes what is computed:
  *   "time_steps" 0|1  record CUDA events around the step launches of each pass (rtm_last_pass_ms);
  *   "pdl"        0|1  programmatic dependent launch between consecutive step kernels (default 1);
- *   "rx"         2|4|8|16|0  rows per thread of the 2D streaming kernel (0 = automatic; T > 1, 2D acoustic only).
+ *   "rx"         2|4|8|16|0  rows per thread of the 2D streaming kernel (0 = automatic; T > 1, 2D acoustic only);
+ *   "resident"   0..3  2D acoustic with time-blocked probing: keep the wavefield in shared memory for a whole time block
+ *                     (one launch per block instead of one per step).  1 (default): when the grid fits ONE thread-block
+ *                     cluster (<= 16 slabs exchanging rows through distributed shared memory; small grids, which are
+ *                     launch-bound otherwise); 2: beyond that also one slab per SM exchanging rows through L2 (measured
+ *                     slower than the streaming kernel at c1); 3: the L2 mode only; 0: never.  Same bits
+ *                     in every mode.
  * Errors: RTM_EINVAL (unknown name / value out of range).
  * Timing experiments that break the results ("dbg" masks, per-block time stamps) exist only in a library built with
  * -DRTM_DEBUG (see the end of this header); the product build has neither.                                */

@@ -11,6 +11,7 @@
 
 #include "../../include/rtm.h"
 #include "acoustic.cuh"
+#include "acoustic2d_resident.cuh"
 #include "acoustic2d_stream.cuh"
 #include "acoustic3d_stream.cuh"
 #include "image.cuh"
@@ -77,6 +78,13 @@ struct rtm_ctx {
     float *smp_w;
     int *offs;
     unsigned long long *dbg_ts;
+    // resident 2D kernel (acoustic2d_resident.cuh): slab decomposition, exchange buffer, step counters
+    struct ResPlan { int nb, groups; size_t smem; } res[2];   // [0] one cluster + DSMEM, [1] exchange through L2; nb = 0: not available
+    float *xbuf;
+    unsigned *flags;
+    int *res_err;
+    unsigned res_ep;          // value of the step counters after the last resident launch
+    int opt_resident;         // option "resident": 0 never, 1 (default) the cluster mode when the grid fits one, 2 also the L2-exchange mode
     void *tmaps;            // 4 CUtensorMaps of the 3D streaming kernel (u ping, u pong, K2, du), device memory
     long long nrows;
     bool have_model, have_probes, have_U, have_V;
@@ -95,6 +103,7 @@ struct rtm_ctx {
 
 static int pick_rx(rtm_ctx *c);
 static int make_tmaps(rtm_ctx *c);
+static int plan_resident(rtm_ctx *c);
 static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace, size_t bytes);
 static size_t stream_smem(const rtm_ctx *c, int rx);
 static long long stream_blocks(const rtm_ctx *c, int rx);
@@ -180,6 +189,10 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t o_of = take(5 * 4096 * 4);   // offsets / (ih, hx, hy) triples, then 512 run records of the tiled xy gather
     size_t o_dbg = take(1024 * 8 * 8);
     size_t o_tm = take(4 * 128);
+    // resident 2D kernel: step counters (one per SM-slab, 128 bytes apart), error word, exchange buffer [2][NB][8][4 nq]
+    const bool res2d = c->ndim == 2 && c->physics == 0 && T > 0;
+    size_t o_fl = take(res2d ? 256 * 128 + 256 : 0);
+    size_t o_xb = take(res2d ? (size_t)2 * 256 * 8 * (size_t)(L.Pz + 4) * 4 : 0);
     if (ctx) {
         char *b = ctx->ws;
         ctx->nf = nf;
@@ -214,6 +227,9 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->offs = (int *)(b + o_of);
         ctx->dbg_ts = (unsigned long long *)(b + o_dbg);
         ctx->tmaps = b + o_tm;
+        ctx->flags = res2d ? (unsigned *)(b + o_fl) : nullptr;
+        ctx->res_err = res2d ? (int *)(b + o_fl + 256 * 128) : nullptr;
+        ctx->xbuf = res2d ? (float *)(b + o_xb) : nullptr;
         ctx->nrows = nrows;
     }
     return off;
@@ -276,6 +292,9 @@ static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace
     CU(cudaMallocHost(&c->h_offs, 5 * 4096 * 4));
     CU(cudaEventCreateWithFlags(&c->offs_done, cudaEventDisableTiming));
     if (cfg->ndim == 3 && cfg->physics == 0 && c->T > 0) return make_tmaps(c);
+    c->opt_resident = 1;
+    c->res_ep = 0;
+    if (cfg->ndim == 2 && cfg->physics == 0 && c->T > 0) return plan_resident(c);
     return RTM_OK;
 }
 
@@ -501,9 +520,17 @@ static int corners_of(const rtm_config &cfg, const Layout &L, const float *xyz, 
     return cnt;
 }
 
+// slab of the resident 2D kernel that owns padded row jx (the first rrem slabs have one row more)
+static int slab_of_row(const rtm_ctx *c, int nb, int jx) {
+    const int rbase = c->L.Px / nb, rrem = c->L.Px % nb;
+    const int big = rrem * (rbase + 1);
+    return jx < big ? jx / (rbase + 1) : rrem + (jx - big) / rbase;
+}
+
 struct PassGeom {
     int ninj, nsmp, nc;
     int bx0, bx1, by0, by1, bz0, bz1;
+    bool res_ok[2];   // the resident 2D kernel's per-slab tables (injection groups, sampled points) can hold this geometry, per mode
 };
 
 // Build injection (row-CSR) and sampling tables on the host and upload them.
@@ -540,12 +567,27 @@ static int build_geometry(rtm_ctx *c, int slot, int ninj, const float *inj_xyz, 
     for (const Tmp &t : tmp) h.row_start[t.row + 1]++;
     for (long long i = 0; i < c->nrows; i++) h.row_start[i + 1] += h.row_start[i];
     for (size_t i = 0; i < tmp.size(); i++) h.ent[i] = {tmp[i].jz, tmp[i].id, tmp[i].w, 0};
+    // resident 2D kernel: do the per-slab tables hold this geometry?  (injection groups = distinct (row, quad) pairs)
+    std::vector<int> per_slab[2];
+    for (int m = 0; m < 2; m++) {
+        g->res_ok[m] = c->res[m].nb > 0;
+        per_slab[m].assign(std::max(1, c->res[m].nb), 0);
+        if (!g->res_ok[m]) continue;
+        long long lrow = -1; int lq = -1;
+        for (const Tmp &t : tmp) {
+            if (t.row != lrow || (t.jz >> 2) != lq) { per_slab[m][slab_of_row(c, c->res[m].nb, (int)t.row)]++; lrow = t.row; lq = t.jz >> 2; }
+        }
+        for (int v : per_slab[m]) g->res_ok[m] = g->res_ok[m] && v <= RS_MAXG;
+        std::fill(per_slab[m].begin(), per_slab[m].end(), 0);
+    }
     for (int s = 0; s < nsmp; s++) {
         if (corners_of(cfg, L, smp_xyz + (size_t)s * nd, co) < 0) return RTM_EINVAL;
         for (int k = 0; k < nc; k++) {
             h.smp_idx[(size_t)s * nc + k] = (int)(L.org + co[k].jx * L.sx + co[k].jy * L.sy + co[k].jz);
             h.smp_w[(size_t)s * nc + k] = co[k].w;
         }
+        for (int m = 0; m < 2; m++)
+            if (g->res_ok[m]) g->res_ok[m] = ++per_slab[m][slab_of_row(c, c->res[m].nb, co[0].jx)] <= RS_MAXS;
     }
     CU(cudaMemcpyAsync(c->row_start, h.row_start, (size_t)(c->nrows + 1) * 4, cudaMemcpyHostToDevice, st));
     if (!tmp.empty())
@@ -592,6 +634,96 @@ static int make_tmaps(rtm_ctx *c) {
         }
     }
     CU(cudaMemcpy(c->tmaps, maps, sizeof maps, cudaMemcpyHostToDevice));
+    return RTM_OK;
+}
+
+// ---- resident 2D kernel: plan and launch (acoustic2d_resident.cuh) ----------------------------------------------------
+static size_t resident_smem(const Layout &L, int rmax) {
+    const int nq = (L.Pz + 3) / 4, spz = nq * 4 + 8;
+    return (size_t)2 * (rmax + 8) * spz * 4 + (size_t)rmax * nq * 16 + (size_t)(RS_MAXG + 1) * (2 * 16 + sizeof(RsGroup)) +
+           (size_t)RS_MAXS * sizeof(RsSample) + (size_t)rmax * nq + 16;
+}
+// Mode 1 (exchange through L2): one slab per SM, the largest NB <= #SM whose slabs have >= 4 rows (a halo comes from ONE
+// neighbour).  Mode 0 (one cluster): the same with NB <= 16 blocks that form one thread-block cluster.  A plan stands if
+// the slabs fit the shared memory of an SM and the threads of a block cover the quad columns.
+static int plan_resident(rtm_ctx *c) {
+    const Layout &L = c->L;
+    c->res[0].nb = c->res[1].nb = 0;
+    int nsm = 0, smem_max = 0;
+    CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->device));
+    CU(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+    const int nq = (L.Pz + 3) / 4;
+    for (int m = 0; m < 2; m++) {
+        const void *fn = m == 0 ? (const void *)acoustic2d_resident_kernel<true> : (const void *)acoustic2d_resident_kernel<false>;
+        for (int cap = m == 0 ? 16 : std::min(nsm, 256); cap >= (m == 0 ? 2 : 1); cap = m == 0 ? cap / 2 : 0) {
+            const int nb = std::min(cap, L.Px / 4);
+            if (nb < 1 || (m == 0 && nb < 2)) break;
+            if (m == 1 ? 2 * nq > RS_THREADS - 32 : nq > RS_THREADS) break;   // mode 1: two sweeping threads per column + the communication warp
+            const int rmax = (L.Px + nb - 1) / nb;
+            if (rmax > RS_MAXROWS) break;
+            const size_t smem = resident_smem(L, rmax);
+            if (smem + 1024 > (size_t)smem_max) break;
+            CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            if (m == 0) {
+                CU(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeClusterDimension;
+                at[0].val.clusterDim.x = (unsigned)nb; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                cudaLaunchConfig_t lc;
+                memset(&lc, 0, sizeof lc);
+                lc.gridDim = dim3((unsigned)nb, 1, 1); lc.blockDim = dim3(RS_THREADS, 1, 1); lc.dynamicSmemBytes = smem;
+                lc.attrs = at; lc.numAttrs = 1;
+                int ncl = 0;
+                if (cudaOccupancyMaxActiveClusters(&ncl, fn, &lc) != cudaSuccess || ncl < 1) { cudaGetLastError(); continue; }   // try a smaller cluster
+            } else {
+                int per_sm = 0;
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, acoustic2d_resident_kernel<false>, RS_THREADS, smem));
+                if (per_sm < 1) break;
+            }
+            c->res[m].nb = nb;
+            c->res[m].groups = m == 0 ? std::max(1, std::min(L.Px / nb, RS_THREADS / nq)) : 2;
+            c->res[m].smem = smem;
+            break;
+        }
+    }
+    CU(cudaMemset(c->flags, 0, 256 * 128 + 256));
+    return RTM_OK;
+}
+
+// nsteps steps starting at time index n0, fields in fld[0][cur] / fld[0][2], history slots hist0, hist0 + pNu, ...
+static int launch_resident(rtm_ctx *c, int mode, const StepArgs &a, int adjoint, int n0, int nsteps, int cur, const PassGeom &g,
+                           const float *d_inj_val, float *d_smp_out, float *hist0, cudaStream_t st) {
+    const Layout &L = c->L;
+    ResidentArgs ra;
+    memset(&ra, 0, sizeof ra);
+    const rtm_ctx::ResPlan &pl = c->res[mode];
+    ra.NB = pl.nb;
+    ra.rbase = L.Px / pl.nb; ra.rrem = L.Px % pl.nb; ra.rmax = ra.rbase + (ra.rrem ? 1 : 0);
+    ra.nq = (L.Pz + 3) / 4; ra.spz = ra.nq * 4 + 8;
+    ra.groups = pl.groups;
+    ra.nsteps = nsteps; ra.n0 = n0; ra.dir = adjoint ? -1 : 1;
+    ra.ninj = g.ninj; ra.inj_base = d_inj_val;
+    ra.smp_base = (d_smp_out != nullptr && g.nsmp > 0) ? d_smp_out : nullptr;
+    ra.hist0 = hist0;
+    ra.u = c->fld[0][cur]; ra.du = c->fld[0][2];
+    ra.xbuf = c->xbuf; ra.flags = c->flags; ra.err = c->res_err;
+    ra.ep0 = c->res_ep;
+    c->res_ep += (unsigned)nsteps;
+    cudaLaunchAttribute at[1];
+    if (mode == 0) {
+        at[0].id = cudaLaunchAttributeClusterDimension;   // one cluster: co-scheduled by construction
+        at[0].val.clusterDim.x = (unsigned)pl.nb; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    } else {
+        at[0].id = cudaLaunchAttributeCooperative;        // all blocks co-resident, or the launch fails: blocks wait for their neighbours
+        at[0].val.cooperative = 1;
+    }
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    lc.gridDim = dim3((unsigned)pl.nb, 1, 1); lc.blockDim = dim3(RS_THREADS, 1, 1);
+    lc.dynamicSmemBytes = pl.smem; lc.stream = st; lc.attrs = at; lc.numAttrs = 1;
+    if (mode == 0) CU(cudaLaunchKernelEx(&lc, acoustic2d_resident_kernel<true>, a, ra));
+    else CU(cudaLaunchKernelEx(&lc, acoustic2d_resident_kernel<false>, a, ra));
+    c->launches++;
     return RTM_OK;
 }
 
@@ -802,6 +934,45 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     if (c->opt_time) CU(cudaEventRecord(c->ev[adjoint][evs][0], st));
     int cur = 0;
     const long long Np = (long long)L.Px * L.Py * L.Pzc;
+#ifdef RTM_DEBUG
+    a.dbg = c->opt_dbg;
+    a.dbg_ts = c->dbg_ts;
+#endif
+    const int res_mode = ((c->opt_resident == 1 || c->opt_resident == 2) && c->res[0].nb > 0 && g.res_ok[0]) ? 0
+                       : (c->opt_resident >= 2 && c->res[1].nb > 0 && g.res_ok[1]) ? 1 : -1;
+    if (res_mode >= 0) {
+        // Resident 2D kernel: one cooperative launch per time block (cut after a step whose field is wanted as a
+        // snapshot), the fields stay in fld[0][0] / fld[0][2]; then the block's history is flushed into the planes.
+        int step = 0;
+        while (step < nt) {
+            const int b = step / T, slot = step % T;
+            int len = std::min(T - slot, nt - step);
+            for (size_t q = 0; q < c->snap_steps.size() && c->snap_out; q++) {
+                const int ss = adjoint ? nt - 1 - c->snap_steps[q] : c->snap_steps[q];
+                if (ss >= step && ss < step + len) len = ss - step + 1;
+            }
+            const int n0 = adjoint ? nt - 1 - step : step;
+            int rc_ = launch_resident(c, res_mode, a, adjoint, n0, len, 0, g, d_inj_val, d_smp_out,
+                                      c->hist + ((size_t)(b & 1) * T + slot) * c->pNu, st);
+            if (rc_) return rc_;
+            step += len;
+            const int nlast = adjoint ? nt - step : step - 1;
+            if (step % T == 0 || step == nt) {
+                const int nfirst = adjoint ? nt - 1 - b * T : b * T;
+                launch_flush(c, c->hist + (size_t)(b & 1) * T * c->pNu, step - b * T, Z + (size_t)nfirst * c->zr, a.fl_zstep, PZ, st);
+            }
+            for (size_t q = 0; q < c->snap_steps.size(); q++)
+                if (c->snap_steps[q] == nlast && c->snap_out) {
+                    unpack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, st>>>(L, c->fld[0][0], c->snap_out + (long long)q * Np);
+                    c->launches++;
+                }
+        }
+        if (c->opt_time) { CU(cudaEventRecord(c->ev[adjoint][evs][1], st)); c->ev_count[adjoint]++; }
+        CU(cudaGetLastError());
+        c->snap_steps.clear();
+        c->snap_out = nullptr;
+        return RTM_OK;
+    }
     for (int step = 0; step < nt; step++) {
         const int n = adjoint ? nt - 1 - step : step;
         const int nprev = adjoint ? n + 1 : n - 1;
@@ -1134,6 +1305,11 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
 #ifdef RTM_DEBUG
     if (!strcmp(name, "dbg")) { c->opt_dbg = value; return RTM_OK; }   // timing experiments only: 1 = no flush role, 2 = no stencil
 #endif
+    if (!strcmp(name, "resident")) {   // 2D acoustic, T > 1: wavefield resident in shared memory for a whole time block
+        if (value < 0 || value > 3) return RTM_EINVAL;
+        c->opt_resident = value;
+        return RTM_OK;
+    }
     if (!strcmp(name, "rx")) {   // rows per thread of the 2D streaming kernel (2|4|8|16); 0 = automatic
         if (!c->rx) return RTM_EINVAL;
         if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16) return RTM_EINVAL;   // the kernel's instances

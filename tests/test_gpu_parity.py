@@ -218,6 +218,24 @@ def test_result_does_not_depend_on_the_time_block(make):
             assert np.array_equal(g[k], ref[k]), (T, k)
 
 
+@pytest.mark.parametrize("mode", [1, 3])
+@pytest.mark.parametrize("n,nb,T", [((70, 61), 8, 16), ((130, 257), 12, 5), ((61, 35), 5, 32), ((640, 120), 20, 32)])
+def test_resident_kernel_is_bit_identical_to_the_streaming_kernel(n, nb, T, mode):
+    """2D acoustic, time-blocked probing: the resident kernel (wavefield in shared memory for a whole time block; slabs
+    exchanging 4 rows with their neighbours -- mode 1: one cluster, through distributed shared memory and a cluster
+    barrier; mode 3: one slab per SM, through L2 and per-slab step counters) performs the same operations in the same
+    order per point as the one-launch-per-step streaming kernel: every output must be equal bit for bit, snapshots in
+    the middle of a time block included.  (640 x 120: many slabs; 61 x 35, nb = 5: slabs of 4 rows, nb % 4 != 0.)"""
+    p = ri.random_acoustic(2, n=n, nb=nb, nt=83, r=6, seed=31, nsrc=3, nrec=9)
+    offs = np.array([-2, 0, 1], np.int32)
+    snaps = [3, 40, 82]
+    a = run_gpu(p, snap_steps=snaps, offsets=offs, probe_block=T, options={"resident": mode})
+    b = run_gpu(p, snap_steps=snaps, offsets=offs, probe_block=T, options={"resident": 0})
+    assert a["launches"] < b["launches"] / 2            # a launch + a flush per time block (+ snapshots), not one per step
+    for k in ("data", "qadj", "Uz", "Vz", "image", "gather", "fsnaps", "asnaps"):
+        assert np.array_equal(a[k], b[k]), k
+
+
 def test_time_block_of_32_steps():
     p2 = ri.random_acoustic(2, n=(70, 61), nb=8, nt=83, r=6, seed=31, nsrc=2, nrec=5)
     check_all(p2, snap_steps=[40, 82], offsets=np.array([-2, 0, 1], np.int32), probe_block=32)
