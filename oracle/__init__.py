@@ -73,8 +73,9 @@ def num_threads() -> int:
 class Coeffs:
     """fp32 coefficient arrays of O1 (canonical padded order)."""
 
-    def __init__(self, K2, damp, epsh=None, delh=None, cosT=None, sinT=None):
+    def __init__(self, K2, damp, epsh=None, delh=None, cosT=None, sinT=None, cosP=None, sinP=None):
         self.K2, self.damp, self.epsh, self.delh, self.cosT, self.sinT = K2, damp, epsh, delh, cosT, sinT
+        self.cosP, self.sinP = cosP, sinP          # 3D TTI: azimuth of the symmetry axis (reading C30)
 
 
 def coeffs(p, vp=None) -> Coeffs:
@@ -90,6 +91,12 @@ def coeffs(p, vp=None) -> Coeffs:
     dh = np.zeros(Np, np.float32) if tti else None
     ct = np.zeros(Np, np.float32) if tti else None
     st = np.zeros(Np, np.float32) if tti else None
+    if tti and p.ndim == 3:
+        cp, sp = np.zeros(Np, np.float32), np.zeros(Np, np.float32)
+        rc = lib.orc_coeffs3(C.byref(c), _fp(vp), _fp(_f32(p.eps)), _fp(_f32(p.delta)), _fp(_f32(p.theta)),
+                             _fp(_f32(p.phi)), _fp(K2), _fp(damp), _fp(eh), _fp(dh), _fp(ct), _fp(st), _fp(cp), _fp(sp))
+        assert rc == 0
+        return Coeffs(K2, damp, eh, dh, ct, st, cp, sp)
     rc = lib.orc_coeffs(C.byref(c), _fp(vp), _fp(_f32(p.eps)), _fp(_f32(p.delta)), _fp(_f32(p.theta)),
                         _fp(K2), _fp(damp), _fp(eh), _fp(dh), _fp(ct), _fp(st))
     assert rc == 0
@@ -121,11 +128,18 @@ def propagate(p, co: Coeffs, adjoint: bool, inj_xyz, inj_val, smp_xyz=None, Z=No
     hist = np.zeros((nt, N) if fields == 1 else (nt, 2, N), np.float64) if want_hist else None
     ss = np.asarray(list(snap_steps), np.int32)
     snaps = np.zeros((len(ss), nf, Np), np.float64) if len(ss) else None
-    fn = lib.orc_propagate if fields == 1 else lib.orc_propagate_pr
-    rc = fn(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
-                           _fp(co.delh), _fp(co.cosT), _fp(co.sinT), C.c_int(ninj), _fp(inj_xyz), _fp(inj_val),
-                           C.c_int(nsmp), _fp(smp_xyz), _fp(out), _fp(Zc), _fp(PZ), _fp(hist),
-                           C.c_int(len(ss)), _fp(ss), _fp(snaps))
+    if p.physics == 1 and p.ndim == 3:
+        assert fields == 1 and co.cosP is not None
+        rc = lib.orc_propagate3(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
+                                _fp(co.delh), _fp(co.cosT), _fp(co.sinT), _fp(co.cosP), _fp(co.sinP), C.c_int(ninj),
+                                _fp(inj_xyz), _fp(inj_val), C.c_int(nsmp), _fp(smp_xyz), _fp(out), _fp(Zc), _fp(PZ),
+                                _fp(hist), C.c_int(len(ss)), _fp(ss), _fp(snaps))
+    else:
+        fn = lib.orc_propagate if fields == 1 else lib.orc_propagate_pr
+        rc = fn(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
+                _fp(co.delh), _fp(co.cosT), _fp(co.sinT), C.c_int(ninj), _fp(inj_xyz), _fp(inj_val),
+                C.c_int(nsmp), _fp(smp_xyz), _fp(out), _fp(Zc), _fp(PZ), _fp(hist),
+                C.c_int(len(ss)), _fp(ss), _fp(snaps))
     if rc != 0:
         raise ValueError("orc_propagate failed rc=%d" % rc)
     return {"samples": out, "PZ": PZ, "hist": hist, "snaps": snaps}
@@ -237,6 +251,9 @@ def tti_H(p, co, which, f):
     c = _cfg(p)
     f = np.ascontiguousarray(f, np.float64).ravel()
     out = np.zeros_like(f)
-    rc = lib.orc_tti_H(C.byref(c), _fp(co.cosT), _fp(co.sinT), C.c_int(which), _fp(f), _fp(out))
+    if p.ndim == 3:
+        rc = lib.orc_tti_H3(C.byref(c), _fp(co.cosT), _fp(co.sinT), _fp(co.cosP), _fp(co.sinP), C.c_int(which), _fp(f), _fp(out))
+    else:
+        rc = lib.orc_tti_H(C.byref(c), _fp(co.cosT), _fp(co.sinT), C.c_int(which), _fp(f), _fp(out))
     assert rc == 0
     return out

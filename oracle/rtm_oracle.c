@@ -2,7 +2,7 @@
  * rtm_oracle.c -- CPU ORACLE.  TEST INFRASTRUCTURE ONLY.
  *
  * A plain, slow, fp64 implementation of what the hot path of arxiv 2201.06914 computes:
- * time-domain FD wave propagation (acoustic 2D/3D, pseudo-acoustic TTI 2D) with the
+ * time-domain FD wave propagation (acoustic 2D/3D, pseudo-acoustic TTI 2D/3D) with the
  * randomized-trace imaging condition accumulated in the time loop (Eq. 3),
  * the image (Eq. 3), the exact zero-lag image from stored history (Eq. 2, in the
  * u.v form -- reading C4 of DESIGN.md) and horizontal subsurface-offset volumes (Eq. 4,
@@ -28,6 +28,8 @@
  * Damped update (C7/C23): the centred scheme solved for the new level, stepped in numpy, to 1e-12 on the whole
  * padded grid; in-layer attenuation exp(-int sigma/c) of the stated profile.  TTI kinematics (C10): homogeneous
  * VTI is faster along x by sqrt(1 + 2 eps); with theta = +30 deg the fast direction is (cos th, -sin th).
+ * 3D TTI (C30; tests/test_oracle_tti3d.py): dot test, H symmetric negative semi-definite, H_perp + H_par = Laplacian for
+ * constant angles, eps = delta = 0 => p == r == acoustic, tilted kinematics (c along n, c sqrt(1+2 eps) along e1, e2).
  * PARITY UNPINNED (free choices no external fact fixes; the implementation is pinned to its stated design, the
  * design itself is a choice): the damping profile shape and strength, the wavelet delay, and imaging the single
  * TTI field (p+r)/2.
@@ -49,7 +51,7 @@ typedef struct {
     int ndim;      /* 2 or 3 */
     int n[3];      /* physical points: 2D uses n[0]=nx, n[1]=nz ; 3D nx,ny,nz */
     int nb;        /* absorbing layer points on every side */
-    int physics;   /* 0 acoustic, 1 TTI (2D only) */
+    int physics;   /* 0 acoustic, 1 TTI (2D: tilt theta; 3D: tilt theta and azimuth phi) */
     int nt;
     int r;
     double h;      /* grid spacing [m]; must be exactly representable as the fp32 the GPU gets */
@@ -119,9 +121,9 @@ static inline int layer_of(const geom *g, int a) { return (g->nd == 2 && a == 1)
  *   TTI: epsh = 1 + 2 eps ; delh = sqrt(1 + 2 min(delta, eps)) ; cos(theta), sin(theta)
  * Outputs: K2,epsh,delh,cosT,sinT [Np] canonical padded order; damp = concat over active axes.
  */
-int orc_coeffs(const orc_cfg *c, const float *vp, const float *eps, const float *delta,
-               const float *theta, float *K2, float *damp, float *epsh, float *delh, float *cosT,
-               float *sinT) {
+static int coeffs_impl(const orc_cfg *c, const float *vp, const float *eps, const float *delta,
+               const float *theta, const float *phi, float *K2, float *damp, float *epsh, float *delh, float *cosT,
+               float *sinT, float *cosP, float *sinP) {
     geom g; make_geom(c, &g);
     double vmax = 0.0;
     for (long i = 0; i < g.N; i++) if (vp[i] > vmax) vmax = vp[i];
@@ -162,10 +164,26 @@ int orc_coeffs(const orc_cfg *c, const float *vp, const float *eps, const float 
                     delh[dst] = (float)sqrt(1.0 + 2.0 * dl);
                     cosT[dst] = (float)cos(th);
                     sinT[dst] = (float)sin(th);
+                    if (phi) {          /* 3D: azimuth of the symmetry axis (reading C30) */
+                        cosP[dst] = (float)cos((double)phi[src]);
+                        sinP[dst] = (float)sin((double)phi[src]);
+                    }
                 }
             }
     for (int a = 0; a < 3; a++) free(sd[a]);
     return 0;
+}
+
+int orc_coeffs(const orc_cfg *c, const float *vp, const float *eps, const float *delta,
+               const float *theta, float *K2, float *damp, float *epsh, float *delh, float *cosT,
+               float *sinT) {
+    return coeffs_impl(c, vp, eps, delta, theta, NULL, K2, damp, epsh, delh, cosT, sinT, NULL, NULL);
+}
+/* 3D TTI (reading C30): the same plus cos / sin of the azimuth phi of the symmetry axis */
+int orc_coeffs3(const orc_cfg *c, const float *vp, const float *eps, const float *delta, const float *theta,
+                const float *phi, float *K2, float *damp, float *epsh, float *delh, float *cosT, float *sinT,
+                float *cosP, float *sinP) {
+    return coeffs_impl(c, vp, eps, delta, theta, phi, K2, damp, epsh, delh, cosT, sinT, cosP, sinP);
 }
 
 /* K1 at padded point (jx,jy,jz) from the fp32 per-axis tables (O1) */
@@ -240,6 +258,74 @@ static inline double dz8(const double *f, long i) {
     return s;
 }
 
+static inline double dy8(const geom *g, const double *f, long i) {
+    double s = 0.0;
+    for (int j = 1; j <= 4; j++) s += W1(j) * (f[i + j * g->sy] - f[i - j * g->sy]);
+    return s;
+}
+
+/* Rotated self-adjoint operators in 3D (reading C30; "TTI", L81 "generalize to 3D").  Symmetry axis
+ *   n  = (sin th cos ph, sin th sin ph, cos th)            (tilt th from the z axis, azimuth ph from the x axis)
+ * and an orthonormal basis of the plane perpendicular to it
+ *   e1 = (cos th cos ph, cos th sin ph, -sin th),   e2 = (-sin ph, cos ph, 0).
+ * With G_v f = v . (Dx f, Dy f, Dz f)  (undivided centred order-8 first derivatives, evaluated on P, zero outside):
+ *   which = 1:  H_par  f = -G_n^T G_n f              = Dx(nx g) + Dy(ny g) + Dz(nz g),          g = G_n f
+ *   which = 0:  H_perp f = -(G_e1^T G_e1 + G_e2^T G_e2) f = Dx(e1x g1 + e2x g2) + Dy(e1y g1 + e2y g2) + Dz(e1z g1),
+ *                                                                                    g1 = G_e1 f, g2 = G_e2 f
+ * (D^T = -D with zeros outside P, reading C8).  For ph = 0 and fields that do not depend on y this is the 2D pair
+ * above; for constant angles H_perp + H_par = Dx Dx + Dy Dy + Dz Dz exactly (e1, e2, n orthonormal).
+ * f, out, t1, t2, t3 live on E; ct, st, cp, sp are [Np] fp32.                                              */
+static void tti_H3(const geom *g, const float *ct, const float *st, const float *cp, const float *sp, int which,
+                   const double *f, double *out, double *t1, double *t2, double *t3) {
+    memset(t1, 0, (size_t)g->NE * sizeof(double));
+    memset(t2, 0, (size_t)g->NE * sizeof(double));
+    memset(t3, 0, (size_t)g->NE * sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (int jx = 0; jx < g->P[0]; jx++)
+        for (int jy = 0; jy < g->P[1]; jy++)
+            for (int jz = 0; jz < g->P[2]; jz++) {
+                long i = eidx(g, jx, jy, jz);
+                long p = pidx(g, jx, jy, jz);
+                double cT = ct[p], sT = st[p], cP = cp[p], sP = sp[p];
+                double fx = dx8(g, f, i), fy = dy8(g, f, i), fz = dz8(f, i);
+                if (which == 1) {
+                    double nx = sT * cP, ny = sT * sP, nz = cT;
+                    double gg = nx * fx + ny * fy + nz * fz;
+                    t1[i] = nx * gg; t2[i] = ny * gg; t3[i] = nz * gg;
+                } else {
+                    double e1x = cT * cP, e1y = cT * sP, e1z = -sT, e2x = -sP, e2y = cP;
+                    double g1 = e1x * fx + e1y * fy + e1z * fz;
+                    double g2 = e2x * fx + e2y * fy;
+                    t1[i] = e1x * g1 + e2x * g2; t2[i] = e1y * g1 + e2y * g2; t3[i] = e1z * g1;
+                }
+            }
+#pragma omp parallel for schedule(static)
+    for (int jx = 0; jx < g->P[0]; jx++)
+        for (int jy = 0; jy < g->P[1]; jy++)
+            for (int jz = 0; jz < g->P[2]; jz++) {
+                long i = eidx(g, jx, jy, jz);
+                out[i] = dx8(g, t1, i) + dy8(g, t2, i) + dz8(t3, i);
+            }
+}
+
+/* test hook: apply the 3D H_perp / H_par to a padded-grid function (pins: symmetry, definiteness, rotation invariance) */
+int orc_tti_H3(const orc_cfg *c, const float *cosT, const float *sinT, const float *cosP, const float *sinP, int which,
+               const double *fP, double *outP) {
+    geom g; make_geom(c, &g);
+    if (c->ndim != 3) return -1;
+    double *f = calloc((size_t)g.NE, sizeof(double)), *o = calloc((size_t)g.NE, sizeof(double));
+    double *t1 = malloc((size_t)g.NE * sizeof(double)), *t2 = malloc((size_t)g.NE * sizeof(double)), *t3 = malloc((size_t)g.NE * sizeof(double));
+    for (int jx = 0; jx < g.P[0]; jx++)
+        for (int jy = 0; jy < g.P[1]; jy++)
+            for (int jz = 0; jz < g.P[2]; jz++) f[eidx(&g, jx, jy, jz)] = fP[pidx(&g, jx, jy, jz)];
+    tti_H3(&g, cosT, sinT, cosP, sinP, which, f, o, t1, t2, t3);
+    for (int jx = 0; jx < g.P[0]; jx++)
+        for (int jy = 0; jy < g.P[1]; jy++)
+            for (int jz = 0; jz < g.P[2]; jz++) outP[pidx(&g, jx, jy, jz)] = o[eidx(&g, jx, jy, jz)];
+    free(f); free(o); free(t1); free(t2); free(t3);
+    return 0;
+}
+
 /* Rotated self-adjoint operators of O5 (2D; symmetry axis (sin th, cos th) in (x,z)):
  *   which = 0:  H_perp f = Dx(cos g) - Dz(sin g),  g = cos Dx f - sin Dz f      (= -G^T G f)
  *   which = 1:  H_par  f = Dx(sin g) + Dz(cos g),  g = sin Dx f + cos Dz f
@@ -307,6 +393,7 @@ int orc_tti_H(const orc_cfg *c, const float *cosT, const float *sinT, int which,
  * Returns 0, or -2 if a position is outside the physical grid.                                   */
 static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
                   const float *epsh, const float *delh, const float *cosT, const float *sinT,
+                  const float *cosP, const float *sinP /* 3D TTI only, else NULL */,
                   int ninj, const float *inj_xyz, const float *inj_val /*[nt][ninj]*/,
                   int nsmp, const float *smp_xyz, double *smp_out /*[nt][nsmp] or NULL*/,
                   const float *Z /*[nt][r] or NULL*/, double *PZ /*[np][r][N] or NULL*/,
@@ -314,7 +401,7 @@ static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float
                   double *snaps, int np /* probed fields: 1, or 2 = p and r apart (TTI) */) {
     geom g; make_geom(c, &g);
     const int d = c->ndim, tti = (c->physics == 1);
-    if (tti && d != 2) return -1;
+    if (tti && d == 3 && (!cosP || !sinP)) return -1;
     if (np != 1 && !(np == 2 && tti)) return -1;
     const int nf = tti ? 2 : 1;
     const int nc = 1 << d;
@@ -337,10 +424,11 @@ static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float
     double *F[2][3];          /* [field][prev,cur,new] on E */
     for (int f = 0; f < 2; f++) for (int k = 0; k < 3; k++)
         F[f][k] = (f < nf) ? calloc((size_t)g.NE, sizeof(double)) : NULL;
-    double *A = NULL, *B = NULL, *t1 = NULL, *t2 = NULL, *ma = NULL, *mb = NULL;
+    double *A = NULL, *B = NULL, *t1 = NULL, *t2 = NULL, *t3 = NULL, *ma = NULL, *mb = NULL;
     if (tti) {
         A = calloc((size_t)g.NE, sizeof(double)); B = calloc((size_t)g.NE, sizeof(double));
         t1 = malloc((size_t)g.NE * sizeof(double)); t2 = malloc((size_t)g.NE * sizeof(double));
+        t3 = malloc((size_t)g.NE * sizeof(double));
         ma = calloc((size_t)g.NE, sizeof(double)); mb = calloc((size_t)g.NE, sizeof(double));
     }
     if (PZ) memset(PZ, 0, sizeof(double) * (size_t)np * (size_t)c->r * (size_t)g.N);
@@ -364,20 +452,27 @@ static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float
             if (adjoint) {     /* pre-mix (O6) */
 #pragma omp parallel for schedule(static)
                 for (int jx = 0; jx < g.P[0]; jx++)
+                    for (int jy = 0; jy < g.P[1]; jy++)
                     for (int jz = 0; jz < g.P[2]; jz++) {
-                        long i = eidx(&g, jx, 0, jz), p = pidx(&g, jx, 0, jz);
+                        long i = eidx(&g, jx, jy, jz), p = pidx(&g, jx, jy, jz);
                         ma[i] = (double)epsh[p] * pc[i] + (double)delh[p] * rc[i];
                         mb[i] = (double)delh[p] * pc[i] + rc[i];
                     }
                 opA = ma; opB = mb;
             }
-            tti_H(&g, cosT, sinT, 0, opA, A, t1, t2);
-            tti_H(&g, cosT, sinT, 1, opB, B, t1, t2);
+            if (d == 2) {
+                tti_H(&g, cosT, sinT, 0, opA, A, t1, t2);
+                tti_H(&g, cosT, sinT, 1, opB, B, t1, t2);
+            } else {
+                tti_H3(&g, cosT, sinT, cosP, sinP, 0, opA, A, t1, t2, t3);
+                tti_H3(&g, cosT, sinT, cosP, sinP, 1, opB, B, t1, t2, t3);
+            }
 #pragma omp parallel for schedule(static)
             for (int jx = 0; jx < g.P[0]; jx++)
+                for (int jy = 0; jy < g.P[1]; jy++)
                 for (int jz = 0; jz < g.P[2]; jz++) {
-                    long i = eidx(&g, jx, 0, jz), p = pidx(&g, jx, 0, jz);
-                    double k1 = K1_at(&g, damp, jx, 0, jz), k2 = K2[p];
+                    long i = eidx(&g, jx, jy, jz), p = pidx(&g, jx, jy, jz);
+                    double k1 = K1_at(&g, damp, jx, jy, jz), k2 = K2[p];
                     double e = epsh[p], dl = delh[p];
                     double ra = adjoint ? A[i] : e * A[i] + dl * B[i];    /* post-mix (O5) */
                     double rb = adjoint ? B[i] : dl * A[i] + B[i];
@@ -443,7 +538,7 @@ static int propagate(const orc_cfg *c, int adjoint, const float *K2, const float
         }
     }
     for (int f = 0; f < 2; f++) for (int k = 0; k < 3; k++) free(F[f][k]);
-    free(A); free(B); free(t1); free(t2); free(ma); free(mb);
+    free(A); free(B); free(t1); free(t2); free(t3); free(ma); free(mb);
     free(iE); free(iW); free(sE); free(sW);
     return 0;
 }
@@ -453,8 +548,18 @@ int orc_propagate(const orc_cfg *c, int adjoint, const float *K2, const float *d
                   int ninj, const float *inj_xyz, const float *inj_val, int nsmp, const float *smp_xyz,
                   double *smp_out, const float *Z, double *PZ /*[r][N]*/, double *hist /*[nt][N]*/, int nsnap,
                   const int *snap_steps, double *snaps) {
-    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
+    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, NULL, NULL, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
                      Z, PZ, hist, nsnap, snap_steps, snaps, 1);
+}
+
+/* 3D pseudo-acoustic TTI (reading C30): the same pass with the rotated operators tti_H3 (tilt and azimuth).        */
+int orc_propagate3(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
+                   const float *epsh, const float *delh, const float *cosT, const float *sinT, const float *cosP,
+                   const float *sinP, int ninj, const float *inj_xyz, const float *inj_val, int nsmp,
+                   const float *smp_xyz, double *smp_out, const float *Z, double *PZ /*[r][N]*/, double *hist /*[nt][N]*/,
+                   int nsnap, const int *snap_steps, double *snaps) {
+    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, cosP, sinP, ninj, inj_xyz, inj_val, nsmp, smp_xyz,
+                     smp_out, Z, PZ, hist, nsnap, snap_steps, snaps, 1);
 }
 
 /* Four compressed arrays for the TTI gradient (Eq. 2-3 applied to the coupled (p, r) system of
@@ -466,7 +571,7 @@ int orc_propagate_pr(const orc_cfg *c, int adjoint, const float *K2, const float
                      int ninj, const float *inj_xyz, const float *inj_val, int nsmp, const float *smp_xyz,
                      double *smp_out, const float *Z, double *PZ /*[2][r][N]*/, double *hist /*[nt][2][N]*/,
                      int nsnap, const int *snap_steps, double *snaps) {
-    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
+    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, NULL, NULL, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
                      Z, PZ, hist, nsnap, snap_steps, snaps, 2);
 }
 

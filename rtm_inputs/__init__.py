@@ -84,7 +84,8 @@ class Problem:
     vp: np.ndarray                # fp32 [n] migration (smoothed) model
     eps: np.ndarray | None = None
     delta: np.ndarray | None = None
-    theta: np.ndarray | None = None   # radians
+    theta: np.ndarray | None = None   # radians: tilt of the symmetry axis from the z axis
+    phi: np.ndarray | None = None     # radians: its azimuth from the x axis (3D TTI only)
     src_xyz: np.ndarray = field(default=None)   # fp32 [nsrc][ndim]
     rec_xyz: np.ndarray = field(default=None)   # fp32 [nrec][ndim]
     wav: np.ndarray = field(default=None)       # fp32 [nt][nsrc]
@@ -310,6 +311,64 @@ def random_tti(n=(40, 36), nb: int = 8, nt: int = 60, r: int = 4, seed: int = 11
     return Problem("rtti", 2, n, h, nb, 1, nt, dt, r, 15.0, vp, vp.copy(), eps=eps.astype(np.float32),
                    delta=delta.astype(np.float32), theta=theta.astype(np.float32),
                    src_xyz=src, rec_xyz=rec, wav=wav, Z=gaussian_probes(nt, r, seed))
+
+
+def random_tti3d(n=(20, 18, 22), nb: int = 6, nt: int = 40, r: int = 4, seed: int = 21, h: float = 10.0,
+                 nsrc: int = 2, nrec: int = 5) -> Problem:
+    """Small random 3D TTI problem (tilt and azimuth fields) with off-grid positions."""
+    rng = np.random.default_rng(seed)
+    vp = (1500.0 + 2000.0 * _smooth_noise(rng, n, 3.0)).astype(np.float32)
+    eps = 0.25 * _smooth_noise(rng, n, 3.0)
+    delta = np.minimum(0.1 * _smooth_noise(rng, n, 3.0), eps)
+    theta = (np.pi / 4) * (2 * _smooth_noise(rng, n, 3.0) - 1)
+    phi = np.pi * (2 * _smooth_noise(rng, n, 3.0) - 1)
+    dt = 0.5 * cfl_dt_tti(h, float(vp.max()), 0.25) * math.sqrt(2.0 / 3.0)      # three axes instead of two
+    L = [(a - 1) * h for a in n]
+    src = np.stack([rng.uniform(0, l, nsrc) for l in L], 1).astype(np.float32)
+    rec = np.stack([rng.uniform(0, l, nrec) for l in L], 1).astype(np.float32)
+    wav = rng.standard_normal((nt, nsrc)).astype(np.float32)
+    return Problem("rtti3", 3, tuple(n), h, nb, 1, nt, dt, r, 15.0, vp, vp.copy(), eps=eps.astype(np.float32),
+                   delta=delta.astype(np.float32), theta=theta.astype(np.float32), phi=phi.astype(np.float32),
+                   src_xyz=src, rec_xyz=rec, wav=wav, Z=gaussian_probes(nt, r, seed))
+
+
+def make_c4_tti(n=(512, 512, 256), nt: int = 3000, r: int = 16, nb: int = 40, h: float = 12.5,
+                rec_stride: int = 2) -> Problem:
+    """configs[4]'s grid, layered model and acquisition with the anisotropy of configs[2] added (SURVEY 8(f) item 4:
+    3D TTI): seeded smooth epsilon in [0, 0.25], delta in [0, 0.1] (<= epsilon), tilt in [-45, 45] deg and azimuth in
+    [-180, 180] deg; isotropic in the top 5 cells; cell-centred source and receivers (C10)."""
+    p = make_c4(n=n, nt=nt, r=r, nb=nb, h=h, rec_stride=rec_stride)
+    rng = np.random.default_rng(SEED0 + 14)
+    nx, ny, nz = n
+    sig = 30.0 * min(1.0, nx / 512.0) + 1.0
+
+    def smooth():       # low-resolution noise, up-sampled by index (a 512 x 512 x 256 Gaussian filter is too slow)
+        c = [max(4, a // 16) for a in n]
+        f = gaussian_filter(rng.standard_normal(c), sig / 16.0 + 0.5, mode="reflect")
+        f -= f.min()
+        f /= max(f.max(), 1e-30)
+        ix = np.minimum(np.arange(nx) * c[0] // nx, c[0] - 1)
+        iy = np.minimum(np.arange(ny) * c[1] // ny, c[1] - 1)
+        iz = np.minimum(np.arange(nz) * c[2] // nz, c[2] - 1)
+        return f[np.ix_(ix, iy, iz)]
+
+    eps = 0.25 * smooth()
+    delta = np.minimum(0.10 * smooth(), eps)
+    theta = (np.pi / 4.0) * (2.0 * smooth() - 1.0)
+    phi = np.pi * (2.0 * smooth() - 1.0)
+    for a in (eps, delta, theta, phi):
+        a[:, :, :5] = 0.0
+    p.name, p.physics = "c4tti", 1
+    p.eps, p.delta, p.theta, p.phi = (a.astype(np.float32) for a in (eps, delta, theta, phi))
+    p.dt = 0.5 * cfl_dt_tti(h, 4000.0, 0.25) * math.sqrt(2.0 / 3.0)
+    p.wav = ricker(nt, p.dt, p.f0)[:, None].copy()
+    Lx, Ly = (nx - 1) * h, (ny - 1) * h
+    p.src_xyz = np.array([[(nx // 2 + 0.5) * h, (ny // 2 + 0.5) * h, 1.5 * h]], np.float32)
+    rx = (np.arange(0, nx - 1, rec_stride) + 0.5) * h
+    ry = (np.arange(0, ny - 1, rec_stride) + 0.5) * h
+    RX, RY = np.meshgrid(rx, ry, indexing="ij")
+    p.rec_xyz = np.stack([RX.ravel(), RY.ravel(), np.full(RX.size, 1.5 * h)], 1).astype(np.float32)
+    return p
 
 
 def random_acoustic(ndim: int = 2, n=(40, 36), nb: int = 8, nt: int = 60, r: int = 4, seed: int = 5,
