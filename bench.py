@@ -51,6 +51,10 @@ def _make_problem(name):
         p = ri.make_c4()
         p.offsets = np.arange(-4, 5, dtype=np.int32)       # a8 on the 3D volume: 9 offsets along x (9 x 268 MB out)
         return p
+    if name == "c4tti":                                   # 3D TTI on configs[4]'s grid (reading C30)
+        p = ri.make_c4_tti()
+        p.offsets = np.arange(-4, 5, dtype=np.int32)
+        return p
     if name == "c0":
         p = ri.make_c0()
         p.offsets = np.arange(-20, 21, dtype=np.int32)
@@ -61,6 +65,7 @@ def _make_problem(name):
 def workload_desc(p):
     return {"workload": {"c3": "configs[1]+configs[3]: 2D acoustic long-offset subsalt + 41-offset gather",
                          "c2": "configs[2]: 2D TTI", "c4": "configs[4]: 3D acoustic",
+                         "c4tti": "configs[4]'s grid with configs[2]'s anisotropy: 3D TTI (SURVEY 8(f) item 4)",
                          "c0": "configs[0]: 2D acoustic small"}.get(p.name, p.name),
             "grid": list(p.n), "nb": p.nb, "padded_points": p.Np, "nt": p.nt, "r": p.r,
             "nrec": int(len(p.rec_xyz)), "nh": 0 if p.offsets is None else int(len(p.offsets)),
@@ -219,6 +224,10 @@ def byte_model(p, T):
     """Algorithmic DRAM bytes of ONE step launch.  2D: the wavefields, du and the coefficient
     arrays are L2-resident (28-66 MB), so only the probe traffic counts; 3D: 20 B per padded point for the fields."""
     fields = 20.0 * p.Np if p.ndim == 3 else 0.0
+    if p.ndim == 3 and p.physics == 1:
+        # three kernels per step: p, r in; 4 angle arrays in; six vector components out and in again; p, r, dp, dr, K2,
+        # epsh, delh in; p', r', dp', dr' out (adjoint: + the mixed pair out and in, epsh / delh read by the mix kernel)
+        fields = 4.0 * p.Np * (2 + 4 + 6 + 6 + 7 + 4)
     if T <= 1:
         return 8.0 * p.r * p.N + fields                       # every probe plane read + written every step
     return 8.0 * p.r * p.N / T + 8.0 * p.N + fields           # planes every T steps + history slot written and read
@@ -226,11 +235,14 @@ def byte_model(p, T):
 
 def op_model(p):
     """Algorithmic fp32 lane operations (add, mul or fma = 1) of one step launch."""
-    per_pt = {(2, 0): 34.0, (3, 0): 50.0, (2, 1): 110.0}[(p.ndim, p.physics)]
+    # 3D TTI: two fields x three first derivatives twice (6 x 3 x 12) + rotations / products (~60) + mixing and updates (~14)
+    per_pt = {(2, 0): 34.0, (3, 0): 50.0, (2, 1): 110.0, (3, 1): 290.0}[(p.ndim, p.physics)]
     return per_pt * p.Np + float(p.r) * p.N                    # stencil + update, and r FMAs per probed point
 
 
 def kernel_name(p, T):
+    if p.physics == 1 and p.ndim == 3:
+        return "tti3d_grad_kernel + tti3d_step_kernel<%d>" % (0 if T <= 1 else 16)
     if p.physics == 1:
         return "tti_step_kernel<%d>" % (0 if T <= 1 else 16 if T > 8 else 8 if T > 4 else 4)
     if T <= 1:
@@ -294,9 +306,9 @@ def run_ours(args):
     # ---- headline: device-resident inputs --------------------------------------------------------------------
     m = make_ctx(T)
     # adjoint input (reading C19): F(true model) - F(migration model), computed on the GPU, untimed
-    m.set_model_from_earth(p.vp_true, p.eps, p.delta, p.theta)
+    m.set_model_from_earth(p.vp_true, p.eps, p.delta, p.theta, p.phi)
     d_true = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
-    m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+    m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta, p.phi)
     d_smooth = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
     din = (d_true - d_smooth).contiguous()
     del d_true, d_smooth
@@ -372,7 +384,7 @@ def run_ours(args):
     if args.variants:
         T2 = 0 if T > 1 else (32 if p.physics == 0 else 16)
         m2 = make_ctx(T2)
-        m2.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        m2.set_model_from_earth(p.vp, p.eps, p.delta, p.theta, p.phi)
         shot2 = shot_on(m2)
         shot2()
         ms2 = timed(shot2, 2)
@@ -384,11 +396,11 @@ def run_ours(args):
     # ---- TTI: the exact gradient's four compressed arrays (reading C29), same schedule and inputs,
     # differenced probes forward: 1 warm-up + 2 timed shots -------------------------------------------------------
     four = None
-    if args.variants and p.physics == 1:
+    if args.variants and p.physics == 1 and p.ndim == 2:
         from paper_2201_06914_b200 import probes_dtt_host
         m4 = make_ctx(T, fields=2)
         m4.set_probes(probes_dtt_host(p.Z, p.dt), p.Z)
-        m4.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        m4.set_model_from_earth(p.vp, p.eps, p.delta, p.theta, p.phi)
         shot4 = shot_on(m4)
         shot4()
         ms4 = timed(shot4, 2) / 2
@@ -501,7 +513,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c0", "c1", "c2", "c4"])
+    ap.add_argument("--workload", default="c4", choices=["c0", "c1", "c2", "c4", "c4tti"])
     ap.add_argument("--probe-block", type=int, default=-1,
                     help="T_b of time-blocked probing (default 32 acoustic, 16 TTI; 0/1 = probe fused into every step)")
     ap.add_argument("--variants", type=int, default=1, help="also time the other probe variant (2 shots)")

@@ -44,7 +44,8 @@ typedef struct {
     float h;        /* grid spacing [m], same on every axis                                       */
     int nb;         /* absorbing-layer points on every side, 0..1024 (any value: the internal z axis is
                        shifted so that the physical grid stays float4-aligned)                      */
-    int physics;    /* 0 isotropic acoustic ; 1 pseudo-acoustic TTI (ndim == 2 only)              */
+    int physics;    /* 0 isotropic acoustic ; 1 pseudo-acoustic TTI (2D: tilt; 3D: tilt + azimuth,
+                       use rtm_coeffs_host3 / rtm_set_model3)                                    */
     int nt;         /* time steps                                                                 */
     double dt;      /* time step [s] (used by rtm_coeffs_host only, which rejects dt <= 0 / non-finite) */
     int r;          /* number of probing vectors, 1..256 (Eq. 1)                    */
@@ -82,10 +83,23 @@ int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const float *h_eps
                     const float *h_theta, float *h_K2, float *h_epsh, float *h_delh, float *h_cos,
                     float *h_sin, float *h_damp1d);
 
+/* 3D TTI ("TTI", L81 "generalize to 3D"; reading C30): the symmetry axis is
+ * n = (sin th cos ph, sin th sin ph, cos th) with tilt th (h_theta) from the z axis and azimuth ph (h_phi) from the x
+ * axis, both canonical [N] host arrays in radians.  As rtm_coeffs_host, plus h_cosp / h_sinp = cos / sin of ph [Np].
+ * Errors: RTM_EINVAL (physics != 1 or ndim != 3, NULL, bad dt).                                                       */
+int rtm_coeffs_host3(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
+                     const float *h_theta, const float *h_phi, float *h_K2, float *h_epsh, float *h_delh,
+                     float *h_cos, float *h_sin, float *h_cosp, float *h_sinp, float *h_damp1d);
+
 /* Load the coefficient arrays (canonical [Np] DEVICE arrays; TTI ones NULL for physics 0) and the
  * per-axis damping tables (HOST) into the workspace's internal (haloed, pitched) layout.         */
 int rtm_set_model(rtm_ctx *ctx, const float *d_K2, const float *d_epsh, const float *d_delh,
                   const float *d_cos, const float *d_sin, const float *h_damp1d, void *cuda_stream);
+
+/* The same for a 3D TTI context (d_cosp, d_sinp: cos / sin of the azimuth, canonical [Np] DEVICE arrays).  A 3D TTI
+ * context rejects rtm_set_model (RTM_EINVAL); every other context rejects this call.                                  */
+int rtm_set_model3(rtm_ctx *ctx, const float *d_K2, const float *d_epsh, const float *d_delh, const float *d_cos,
+                   const float *d_sin, const float *d_cosp, const float *d_sinp, const float *h_damp1d, void *cuda_stream);
 
 /* Probing matrices Z (reading C1/C2: E[z z^T] = I, drawn by the caller), device
  * arrays [nt][r]; row n probes the field computed by step n (reading C6).  Zf is used by the
@@ -168,7 +182,8 @@ int rtm_export_probes(rtm_ctx *ctx, int which, float *d_out, void *cuda_stream);
 /* Ask the NEXT pass to copy the wavefield(s) right after the listed steps (incl. injection) into
  * d_out [nsnap][nf][Np] canonical (nf = 1 acoustic, 2 TTI: p then r).  nsnap = 0 clears.          */
 int rtm_set_snapshots(rtm_ctx *ctx, int nsnap, const int *h_steps, float *d_out);
-/* Internal coefficient array in canonical [Np] order: which = 0 K2, 1 epsh, 2 delh, 3 cos, 4 sin. */
+/* Internal coefficient array in canonical [Np] order: which = 0 K2, 1 epsh, 2 delh, 3 cos, 4 sin (tilt), 5 cos, 6 sin
+ * (azimuth, 3D TTI). */
 int rtm_export_coeff(rtm_ctx *ctx, int which, float *d_out, void *cuda_stream);
 /* Number of kernels this context has launched so far (bench.py's gpu_launches).                  */
 long long rtm_launch_count(const rtm_ctx *ctx);

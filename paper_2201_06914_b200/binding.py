@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "csrc", "librtm.so")
 _lib = None
 
-EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_set_model",
+EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_coeffs_host3", "rtm_set_model", "rtm_set_model3",
            "rtm_set_probes", "rtm_probes_dtt_host", "rtm_probes_qr_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_image", "rtm_offset_gather",
            "rtm_offset_gather_xy",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
@@ -53,6 +53,8 @@ def load_library():
     lib.rtm_destroy.restype = None
     lib.rtm_coeffs_host.argtypes = [cfgp] + [vp] * 10
     lib.rtm_set_model.argtypes = [vp] * 8
+    lib.rtm_coeffs_host3.argtypes = [cfgp] + [vp] * 13
+    lib.rtm_set_model3.argtypes = [vp] * 10
     lib.rtm_set_probes.argtypes = [vp] * 4
     lib.rtm_probes_dtt_host.argtypes = [ip, ip, C.c_double, vp, vp]
     lib.rtm_probes_qr_host.argtypes = [ip, ip, ip, vp, vp, vp]
@@ -133,6 +135,21 @@ def coeffs_host(cfg: RtmConfig, vp, eps=None, delta=None, theta=None):
     _check(lib.rtm_coeffs_host(C.byref(cfg), _hp(vp), _hp(eps), _hp(delta), _hp(theta), _hp(K2),
                                _hp(outs[0]), _hp(outs[1]), _hp(outs[2]), _hp(outs[3]), _hp(damp)))
     return K2, outs[0], outs[1], outs[2], outs[3], damp
+
+
+def coeffs_host3(cfg: RtmConfig, vp, eps, delta, theta, phi):
+    """rtm_coeffs_host3 (3D TTI): (K2, epsh, delh, cos th, sin th, cos ph, sin ph, damp1d) as numpy fp32 arrays."""
+    lib = load_library()
+    n = [cfg.n[i] for i in range(3)]
+    P = [a + 2 * cfg.nb for a in n]
+    Np = int(np.prod(P))
+    f32 = lambda a: np.ascontiguousarray(a, np.float32)
+    vp, eps, delta, theta, phi = (f32(a) for a in (vp, eps, delta, theta, phi))
+    outs = [np.empty(Np, np.float32) for _ in range(7)]
+    damp = np.empty(sum(P), np.float32)
+    _check(lib.rtm_coeffs_host3(C.byref(cfg), _hp(vp), _hp(eps), _hp(delta), _hp(theta), _hp(phi),
+                                *[_hp(o) for o in outs], _hp(damp)))
+    return tuple(outs) + (damp,)
 
 
 def probes_qr_host(D, Z):
@@ -232,7 +249,14 @@ class Rtm:
         return None if tens is None else C.c_void_p(tens.data_ptr())
 
     # -- API ------------------------------------------------------------------------------------------
-    def set_model_from_earth(self, vp, eps=None, delta=None, theta=None):
+    def set_model_from_earth(self, vp, eps=None, delta=None, theta=None, phi=None):
+        if self.physics == 1 and self.ndim == 3:            # 3D TTI: tilt and azimuth (reading C30)
+            K2, eh, dh, cs, sn, cp, sp, damp = coeffs_host3(self.cfg, vp, eps, delta, theta, phi)
+            d = [self._dev(a) for a in (K2, eh, dh, cs, sn, cp, sp)]
+            damp = np.ascontiguousarray(damp, np.float32)
+            _check(self.lib.rtm_set_model3(self.ctx, *[self._ptr(x) for x in d], _hp(damp), self._stream()))
+            self._keep = [d, damp]
+            return K2, eh, dh, cs, sn, damp, cp, sp
         K2, eh, dh, cs, sn, damp = coeffs_host(self.cfg, vp, eps, delta, theta)
         self.set_model(K2, eh, dh, cs, sn, damp)
         return K2, eh, dh, cs, sn, damp

@@ -45,6 +45,8 @@ struct StepArgs {
     float *n0, *n1;         // new field(s)
     float *d0, *d1;         // increment(s) du = u_cur - u_prev, updated in place
     const float *K2, *epsh, *delh, *cs, *sn;
+    const float *cp, *sp;   // 3D TTI: cos / sin of the azimuth (cs, sn: of the tilt)
+    float *F[6];            // 3D TTI: the six intermediate vector components (tti3d.cuh)
     const float *dampx, *dampy, *dampz;
     const float *k1x, *k1y, *k1z;   // per-axis K1 tables: k1a[j] = (1 - damp_a[j]) / (1 + damp_a[j])
     int adjoint;

@@ -16,6 +16,7 @@
 #include "acoustic3d_stream.cuh"
 #include "image.cuh"
 #include "tti.cuh"
+#include "tti3d.cuh"
 
 using namespace rtm;
 
@@ -66,6 +67,7 @@ struct rtm_ctx {
     float *fields_base;
     size_t fields_bytes;
     float *K2, *epsh, *delh, *cs, *sn;
+    float *cp, *sp, *F[6];   // 3D TTI
     float *dampx, *dampy, *dampz;
     float *k1x, *k1y, *k1z;
     float *Uz, *Vz, *Zf, *Za, *hist;
@@ -117,7 +119,6 @@ static bool valid_cfg(const rtm_config *c) {
     if (!(c->h > 0.f) || !std::isfinite(c->h)) return false;
     if (c->nb < 0 || c->nb > 1024) return false;
     if (c->physics != 0 && c->physics != 1) return false;
-    if (c->physics == 1 && c->ndim != 2) return false;
     if (c->nt < 1 || c->r < 1 || c->r > 256 || c->max_pts < 1) return false;
     // time blocks of up to 16 steps; the acoustic streaming kernels have the registers for 32 history values per
     // flush-role thread, the TTI kernel (64 registers) has not
@@ -125,7 +126,7 @@ static bool valid_cfg(const rtm_config *c) {
     if (c->probe_block > 16 && c->r > 128) return false;   // staging of the 32 Z rows in the final flush kernel
     // four compressed arrays for the TTI gradient (reading C29): TTI only
     if (c->probe_fields != 0 && c->probe_fields != 1 && c->probe_fields != 2) return false;
-    if (c->probe_fields == 2 && c->physics != 1) return false;
+    if (c->probe_fields == 2 && (c->physics != 1 || c->ndim != 2)) return false;
     return true;
 }
 
@@ -137,7 +138,7 @@ static void make_layout(const rtm_config *c, Layout *L) {
     L->nz = c->ndim == 3 ? c->n[2] : c->n[1];
     L->nb = c->nb;
     L->nby = c->ndim == 3 ? c->nb : 0;
-    L->H = c->physics == 1 ? 8 : 4;
+    L->H = (c->physics == 1 && c->ndim == 2) ? 8 : 4;   // 2D TTI: two chained derivatives inside one tile; 3D TTI: separate kernels
     L->Hy = c->ndim == 3 ? L->H : 0;
     L->Px = L->nx + 2 * c->nb;
     L->Py = L->ny + 2 * L->nby;
@@ -171,6 +172,9 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
     size_t fields_bytes = off - o_fields;
     size_t o_K2 = take(fb), o_e = 0, o_d = 0, o_c = 0, o_s = 0;
     if (nf == 2) { o_e = take(fb); o_d = take(fb); o_c = take(fb); o_s = take(fb); }
+    const bool tti3 = nf == 2 && c->ndim == 3;
+    size_t o_cp = 0, o_sp = 0, o_F[6] = {0, 0, 0, 0, 0, 0};
+    if (tti3) { o_cp = take(fb); o_sp = take(fb); for (int k = 0; k < 6; k++) o_F[k] = take(fb); }
     size_t o_dx = take((size_t)(L.Px + 32) * 4), o_dy = take((size_t)(L.Py + 8) * 4), o_dz = take((size_t)(L.Pz + 8) * 4);
     size_t o_kx = take((size_t)(L.Px + 32) * 4), o_ky = take((size_t)(L.Py + 8) * 4), o_kz = take((size_t)(L.Pz + 8) * 4);
     const int rp = c->probe_fields == 2 ? 2 * c->r : c->r;
@@ -205,6 +209,9 @@ static size_t carve(const rtm_config *c, const Layout &L, rtm_ctx *ctx) {
         ctx->delh = nf == 2 ? (float *)(b + o_d) : nullptr;
         ctx->cs = nf == 2 ? (float *)(b + o_c) : nullptr;
         ctx->sn = nf == 2 ? (float *)(b + o_s) : nullptr;
+        ctx->cp = tti3 ? (float *)(b + o_cp) : nullptr;
+        ctx->sp = tti3 ? (float *)(b + o_sp) : nullptr;
+        for (int k = 0; k < 6; k++) ctx->F[k] = tti3 ? (float *)(b + o_F[k]) : nullptr;
         ctx->dampx = (float *)(b + o_dx);
         ctx->dampy = (float *)(b + o_dy);
         ctx->dampz = (float *)(b + o_dz);
@@ -315,10 +322,11 @@ extern "C" void rtm_destroy(rtm_ctx *c) {
 }
 
 // ---- O1: coefficients on the host (fp64, one rounding to fp32) ---------------------------------
-extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
-                               const float *h_theta, float *h_K2, float *h_epsh, float *h_delh, float *h_cos,
-                               float *h_sin, float *h_damp1d) {
+static int coeffs_host_impl(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
+                            const float *h_theta, const float *h_phi, float *h_K2, float *h_epsh, float *h_delh,
+                            float *h_cos, float *h_sin, float *h_cosp, float *h_sinp, float *h_damp1d) {
     if (!valid_cfg(cfg) || !h_vp || !h_K2 || !h_damp1d) return RTM_EINVAL;
+    if (cfg->physics == 1 && cfg->ndim == 3 && (!h_phi || !h_cosp || !h_sinp)) return RTM_EINVAL;   // 3D TTI needs the azimuth
     if (!(cfg->dt > 0.0) || !std::isfinite(cfg->dt)) return RTM_EINVAL;   // K2 and the damping tables would be 0 or NaN
     const bool tti = cfg->physics == 1;
     if (tti && (!h_eps || !h_delta || !h_theta || !h_epsh || !h_delh || !h_cos || !h_sin)) return RTM_EINVAL;
@@ -367,9 +375,24 @@ extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const f
                     h_delh[d] = (float)std::sqrt(1.0 + 2.0 * dl);
                     h_cos[d] = (float)std::cos(th);
                     h_sin[d] = (float)std::sin(th);
+                    if (h_phi) {
+                        h_cosp[d] = (float)std::cos((double)h_phi[s]);
+                        h_sinp[d] = (float)std::sin((double)h_phi[s]);
+                    }
                 }
             }
     return RTM_OK;
+}
+extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
+                               const float *h_theta, float *h_K2, float *h_epsh, float *h_delh, float *h_cos,
+                               float *h_sin, float *h_damp1d) {
+    return coeffs_host_impl(cfg, h_vp, h_eps, h_delta, h_theta, nullptr, h_K2, h_epsh, h_delh, h_cos, h_sin, nullptr, nullptr, h_damp1d);
+}
+extern "C" int rtm_coeffs_host3(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
+                                const float *h_theta, const float *h_phi, float *h_K2, float *h_epsh, float *h_delh,
+                                float *h_cos, float *h_sin, float *h_cosp, float *h_sinp, float *h_damp1d) {
+    if (!cfg || cfg->physics != 1 || cfg->ndim != 3) return RTM_EINVAL;
+    return coeffs_host_impl(cfg, h_vp, h_eps, h_delta, h_theta, h_phi, h_K2, h_epsh, h_delh, h_cos, h_sin, h_cosp, h_sinp, h_damp1d);
 }
 
 // ---- reading C4: second time difference moved from the wavefield onto the probes (host, fp64) ------------
@@ -433,12 +456,13 @@ static int launch_pack(rtm_ctx *c, const float *src, float *dst, cudaStream_t st
     return RTM_OK;
 }
 
-extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh, const float *d_delh,
-                             const float *d_cos, const float *d_sin, const float *h_damp1d, void *stream) {
+static int set_model_impl(rtm_ctx *c, const float *d_K2, const float *d_epsh, const float *d_delh, const float *d_cos,
+                          const float *d_sin, const float *d_cosp, const float *d_sinp, const float *h_damp1d, void *stream) {
     if (!c || !d_K2 || !h_damp1d) return RTM_EINVAL;
     DeviceGuard guard(c->device);
     const bool tti = c->cfg.physics == 1;
     if (tti && (!d_epsh || !d_delh || !d_cos || !d_sin)) return RTM_EINVAL;
+    if (tti && c->cfg.ndim == 3 && (!d_cosp || !d_sinp)) return RTM_EINVAL;   // 3D TTI: use rtm_set_model3
     cudaStream_t st = (cudaStream_t)stream;
     const Layout &L = c->L;
     // zero everything up to the probe planes once (halo of fields and coefficients stays zero)
@@ -450,6 +474,10 @@ extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh,
         if ((rc = launch_pack(c, d_delh, c->delh, st))) return rc;
         if ((rc = launch_pack(c, d_cos, c->cs, st))) return rc;
         if ((rc = launch_pack(c, d_sin, c->sn, st))) return rc;
+        if (c->cfg.ndim == 3) {
+            if ((rc = launch_pack(c, d_cosp, c->cp, st))) return rc;
+            if ((rc = launch_pack(c, d_sinp, c->sp, st))) return rc;
+        }
     }
     // small tables: pageable source, the copy is staged before the call returns
     const float *t = h_damp1d;
@@ -469,6 +497,16 @@ extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh,
     c->have_model = true;
     c->have_U = c->have_V = false;
     return RTM_OK;
+}
+
+extern "C" int rtm_set_model(rtm_ctx *c, const float *d_K2, const float *d_epsh, const float *d_delh,
+                             const float *d_cos, const float *d_sin, const float *h_damp1d, void *stream) {
+    return set_model_impl(c, d_K2, d_epsh, d_delh, d_cos, d_sin, nullptr, nullptr, h_damp1d, stream);
+}
+extern "C" int rtm_set_model3(rtm_ctx *c, const float *d_K2, const float *d_epsh, const float *d_delh, const float *d_cos,
+                              const float *d_sin, const float *d_cosp, const float *d_sinp, const float *h_damp1d, void *stream) {
+    if (!c || c->cfg.physics != 1 || c->cfg.ndim != 3) return RTM_EINVAL;
+    return set_model_impl(c, d_K2, d_epsh, d_delh, d_cos, d_sin, d_cosp, d_sinp, h_damp1d, stream);
 }
 
 extern "C" int rtm_set_probes(rtm_ctx *c, const float *d_Zf, const float *d_Za, void *stream) {
@@ -730,7 +768,11 @@ static int launch_resident(rtm_ctx *c, int mode, const StepArgs &a, int adjoint,
 // ---- one propagation pass (a1-a6) ---------------------------------------------------------------
 static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
     const Layout &L = c->L;
-    if (c->cfg.physics == 1) {
+    if (c->cfg.physics == 1 && c->cfg.ndim == 3) {
+        *grid = dim3((L.Pz + 127) / 128, (L.Py + 7) / 8, L.Px);
+        *block = dim3(32, 8, 1);
+        *smem = 0;
+    } else if (c->cfg.physics == 1) {
         *grid = dim3((L.Pz + TTI_TZ - 1) / TTI_TZ, (L.Px + TTI_TX - 1) / TTI_TX, 1);
         *block = dim3(16, 16, 1);
         *smem = std::max<size_t>((size_t)TTI_SMEM, (size_t)tm_of(c->T) * c->zr * 4);
@@ -833,7 +875,12 @@ static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, 
 static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     const unsigned nb = a.fl_blocks + grid.x * grid.y * grid.z;
     const int tm = tm_of(c->T);
-    if (c->cfg.physics == 1) {
+    if (c->cfg.physics == 1 && c->cfg.ndim == 3) {   // mix (adjoint), rotated gradients, divergence + update
+        int rc = 0;
+        if (a.adjoint && (rc = launch_ex(c, tti3d_mix_kernel, a, nb, block, 0, st))) return rc;
+        if ((rc = launch_ex(c, tti3d_grad_kernel, a, nb, block, 0, st))) return rc;
+        return tm == 0 ? launch_ex(c, tti3d_step_kernel<0>, a, nb, block, 0, st) : launch_ex(c, tti3d_step_kernel<16>, a, nb, block, 0, st);
+    } else if (c->cfg.physics == 1) {
         switch (tm) {
             case 0: return a.two ? launch_ex(c, tti_step_kernel<0, true>, a, nb, block, smem, st)
                                  : launch_ex(c, tti_step_kernel<0>, a, nb, block, smem, st);
@@ -895,6 +942,9 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
     memset(&a, 0, sizeof a);
     a.L = L;
     a.K2 = c->K2; a.epsh = c->epsh; a.delh = c->delh; a.cs = c->cs; a.sn = c->sn;
+    a.cp = c->cp; a.sp = c->sp;
+    for (int k = 0; k < 6; k++) a.F[k] = c->F[k];
+    const bool tti3 = cfg.physics == 1 && d == 3;   // three kernels per step, no in-launch flush role: flush at the end of a time block
     a.dampx = c->dampx; a.dampy = c->dampy; a.dampz = c->dampz;
     a.k1x = c->k1x; a.k1y = c->k1y; a.k1z = c->k1z;
     a.adjoint = adjoint;
@@ -990,7 +1040,7 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
             // previous block is flushed in len_b slices, one per step launch
             const int b = step / T, slot = step % T;
             a.hist = c->hist + ((size_t)(b & 1) * T + slot) * c->pNu;
-            if (b >= 1) {
+            if (b >= 1 && !tti3) {
                 const int len_b = std::min(T, nt - b * T);
                 const int pb = b - 1;
                 const int nfirst = adjoint ? nt - 1 - pb * T : pb * T;
@@ -1015,6 +1065,11 @@ static int run_pass(rtm_ctx *c, int adjoint, const PassGeom &g, const float *d_i
 #endif
         { int rc_ = launch_step(c, a, grid, block, smem, st); if (rc_) return rc_; }
         cur ^= 1;
+        if (tti3 && T && (step + 1) % T == 0 && step != nt - 1) {
+            const int fb = step / T;
+            const int nfirst = adjoint ? nt - 1 - fb * T : fb * T;
+            launch_flush(c, c->hist + (size_t)(fb & 1) * T * c->pNu, T, Z + (size_t)nfirst * c->zr, a.fl_zstep, PZ, st);
+        }
         if (T && step == nt - 1) {   // the last time block has no following steps to hide behind
             const int fb = step / T, lenf = nt - fb * T;
             const int nfirst = adjoint ? nt - 1 - fb * T : fb * T;
@@ -1258,10 +1313,10 @@ extern "C" int rtm_set_snapshots(rtm_ctx *c, int nsnap, const int *h_steps, floa
 }
 
 extern "C" int rtm_export_coeff(rtm_ctx *c, int which, float *d_out, void *stream) {
-    if (!c || !d_out || which < 0 || which > 4) return RTM_EINVAL;
+    if (!c || !d_out || which < 0 || which > 6) return RTM_EINVAL;
     DeviceGuard guard(c->device);
     if (!c->have_model) return RTM_ESTATE;
-    const float *src[5] = {c->K2, c->epsh, c->delh, c->cs, c->sn};
+    const float *src[7] = {c->K2, c->epsh, c->delh, c->cs, c->sn, c->cp, c->sp};
     if (!src[which]) return RTM_EINVAL;
     const long long Np = (long long)c->L.Px * c->L.Py * c->L.Pzc;
     unpack_field_kernel<<<(unsigned)((Np + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c->L, src[which], d_out);

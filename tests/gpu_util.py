@@ -53,7 +53,7 @@ def run_gpu(p, snap_steps=(), din=None, offsets=None, want_qadj=True, probe_bloc
     m = Rtm.from_problem(p, probe_block=probe_block)
     for k, v in (options or {}).items():
         m.set_option(k, v)
-    coef = m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+    coef = m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta, p.phi)
     m.set_probes(p.Z)
     out = {"coef": coef}
     sn = m.set_snapshots(list(snap_steps)) if len(snap_steps) else None

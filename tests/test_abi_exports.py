@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol():
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     hdr = re.sub(r"#ifdef RTM_DEBUG.*?#endif", "", hdr, flags=re.S)      # timing experiments: -DRTM_DEBUG builds only
     assert not hasattr(lib, "rtm_debug_stamps")                          # the product library has no debug switches
-    declared = sorted(set(re.findall(r"\b(rtm_[a-z_]+)\s*\(", hdr)))
+    declared = sorted(set(re.findall(r"\b(rtm_[a-z0-9_]+)\s*\(", hdr)))
     assert len(declared) >= 15
     for name in declared:
         assert hasattr(lib, name), name
@@ -93,6 +93,18 @@ def test_host_coefficients_match_oracle_bitwise():
         if p.physics == 1:
             for a, b in ((eh, co.epsh), (dh, co.delh), (cs, co.cosT), (sn, co.sinT)):
                 assert np.array_equal(a, b)
+
+
+def test_host_coefficients_3d_tti_match_oracle_bitwise():
+    _build()
+    from paper_2201_06914_b200 import binding as B
+    p = ri.random_tti3d(n=(11, 9, 10), nb=3, nt=5)
+    cfg = B.make_config(p.ndim, p.n, p.h, p.nb, p.physics, p.nt, p.dt, p.r, 8)
+    K2, eh, dh, cs, sn, cp, sp, damp = B.coeffs_host3(cfg, p.vp, p.eps, p.delta, p.theta, p.phi)
+    co = orc.coeffs(p)
+    for a, b in ((K2, co.K2), (damp, co.damp), (eh, co.epsh), (dh, co.delh), (cs, co.cosT), (sn, co.sinT), (cp, co.cosP), (sp, co.sinP)):
+        assert np.array_equal(a, b)
+    assert B.workspace_bytes(B.make_config(3, p.n, p.h, p.nb, 1, p.nt, p.dt, p.r, 8, probe_fields=2)) == 0    # four-array mode: 2D TTI only
 
 
 def test_coeffs_host_rejects_bad_time_step_and_spacing():

@@ -71,7 +71,7 @@ def test_create_errors():
     host = np.zeros(need + 256, np.uint8)
     hp = (host.ctypes.data + 255) // 256 * 256
     assert lib.rtm_create(C.byref(cfg), hp, need, C.byref(h)) == -1                          # host pointer
-    for bad in (dict(nb=-1), dict(nb=1025), dict(ndim=4), dict(physics=1, ndim=3), dict(r=0), dict(nt=0)):
+    for bad in (dict(nb=-1), dict(nb=1025), dict(ndim=4), dict(r=0), dict(nt=0)):
         c2 = B.make_config(bad.get("ndim", 2), (20, 20, 20), 10.0, bad.get("nb", 4), bad.get("physics", 0),
                            bad.get("nt", 5), 1e-3, bad.get("r", 2), 4)
         assert B.workspace_bytes(c2) == 0

@@ -61,6 +61,16 @@ def test_layer_thickness_need_not_be_a_multiple_of_4(nb):
     check_all(q, snap_steps=[49], offsets=np.array([-1, 0, 3], np.int32), probe_block=8 if nb % 2 else 0)
 
 
+@pytest.mark.parametrize("n,nb,r,T", [((20, 18, 22), 6, 4, 0), ((21, 9, 131), 4, 3, 0), ((37, 19, 40), 5, 5, 8),
+                                      ((40, 23, 70), 8, 4, 16)])
+def test_tti3d_random_offgrid(n, nb, r, T):
+    """3D pseudo-acoustic TTI (reading C30): random tilt and azimuth fields, off-grid sources and
+    receivers, ragged tiles in y and z, nb not a multiple of 4, per-step fused and time-blocked probing (nt = 45 is not a
+    multiple of T)."""
+    p = ri.random_tti3d(n=n, nb=nb, nt=45, r=r, seed=6, nsrc=2, nrec=6)
+    check_all(p, snap_steps=[10, 44], offsets=np.array([-2, 0, 1], np.int32), probe_block=T)
+
+
 def test_c1_cropped():
     p = ri.make_c3(n=(256, 200), nt=600, r=32, nb=80)
     import oracle as orc
@@ -150,6 +160,7 @@ def test_gather_h0_equals_image_bitwise():
     lambda: ri.random_acoustic(2, n=(48, 40), nb=8, nt=100, seed=1),
     lambda: ri.random_acoustic(3, n=(16, 14, 18), nb=4, nt=50, seed=2),
     lambda: ri.random_tti(n=(44, 40), nb=8, nt=100, seed=3),
+    lambda: ri.random_tti3d(n=(17, 15, 18), nb=4, nt=40, seed=3),
 ])
 def test_dot_product_on_gpu(make):
     """north_star check 3: <F q, d> = <q, F^T d> to 1e-5 in fp32."""
