@@ -30,6 +30,7 @@ constexpr int RS_THREADS = 512;
 constexpr int RS_MAXG = 255;      // injection groups (row, quad) per block (index + 1 fits a byte)
 constexpr int RS_MAXS = 256;      // sampled points per block
 constexpr int RS_MAXROWS = 64;    // rows per slab the tables are sized for
+constexpr int RS_MAXE = 256;      // injection entries per block (cached in shared memory)
 
 struct ResidentArgs {
     int NB;                 // blocks = slabs
@@ -95,8 +96,11 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
     float *U0 = rs_smem;                                   // [urows][spz]
     float *U1 = U0 + urows * spz;
     float *D = U1 + urows * spz;                           // [rmax][nq4]
-    float4 *staged = reinterpret_cast<float4 *>(D + ra.rmax * nq4);          // [2][RS_MAXG + 1]: this step's / the next step's amounts
-    RsGroup *grp = reinterpret_cast<RsGroup *>(staged + 2 * (RS_MAXG + 1));   // [RS_MAXG]
+    float *Ks = D + ra.rmax * nq4;                         // CL only: K2 of the slab [rmax][nq4] (a small grid has the room)
+    float4 *staged = reinterpret_cast<float4 *>(Ks + (CL ? ra.rmax * nq4 : 0));   // [RS_MAXG + 1]: this step's injection amounts
+    InjEntry *ecache = reinterpret_cast<InjEntry *>(staged + RS_MAXG + 1);   // [RS_MAXE]: the slab's injection entries
+    float *vbuf = reinterpret_cast<float *>(ecache + RS_MAXE);              // [2][RS_MAXE]: their values for this / the next step (cp.async)
+    RsGroup *grp = reinterpret_cast<RsGroup *>(vbuf + 2 * RS_MAXE);          // [RS_MAXG]
     RsSample *smp = reinterpret_cast<RsSample *>(grp + RS_MAXG + 1);          // [RS_MAXS]
     unsigned char *gmap = reinterpret_cast<unsigned char *>(smp + RS_MAXS);   // [rmax][nq]: group index + 1
     __shared__ int s_ngrp, s_nsmp;
@@ -119,6 +123,13 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
         const int lr = i / nq, col = i - lr * nq;
         st4(D + lr * nq4 + col * 4, ld4(ra.du + L.org + (long long)(r0 + lr) * L.sx + col * 4));
     }
+    if (CL)
+        for (int i = tid; i < R * nq; i += RS_THREADS) {
+            const int lr = i / nq, col = i - lr * nq;
+            st4(Ks + lr * nq4 + col * 4, ld4(a.K2 + L.org + (long long)(r0 + lr) * L.sx + col * 4));
+        }
+    const int ebase = a.row_start[r0], nent_b = min(a.row_start[r0 + R] - ebase, RS_MAXE);   // the host checked the cap
+    for (int i = tid; i < nent_b; i += RS_THREADS) ecache[i] = a.ent[ebase + i];
     // injection groups: the entries of a row are sorted by jz, so the entries of one quad are contiguous; one thread
     // per row counts its groups, a serial prefix over <= RS_MAXROWS rows places them (deterministic order)
     if (tid < R) {
@@ -222,24 +233,34 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
     const unsigned *lf = b > 0 ? ra.flags + 32 * (b - 1) : nullptr, *rf = b + 1 < ra.NB ? ra.flags + 32 * (b + 1) : nullptr;
     const unsigned hbytes = (unsigned)((lf ? 4 : 0) + (rf ? 4 : 0)) * (unsigned)nq4 * 4u;
 
-    // injection amounts of a step: v = sum_i scale w_i val_i per lane of the quad, in entry order (C27)
-    auto stage = [&](int n, int buf) {
+    // The values of the slab's injection entries for step n travel by cp.async (4 bytes each) into vbuf[buf] while the
+    // previous step is swept; stage() then forms the amounts v = sum_i scale w_i val_i per lane of each (row, quad) group,
+    // in entry order (C27), from shared memory only: nothing on the critical path of a step waits for L2.
+    auto fetch_values = [&](int n, int buf) {
+        const float *val = ra.inj_base + (size_t)n * ra.ninj;
+        for (int e = tid; e < nent_b; e += RS_THREADS) {
+            const unsigned dsts = smem_u32(vbuf + buf * RS_MAXE + e);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dsts), "l"(val + ecache[e].id) : "memory");
+        }
+        cp_async_commit();
+    };
+    auto stage = [&](int buf) {
         if (tid < ngrp) {
             const RsGroup g = grp[tid];
-            const float *val = ra.inj_base + (size_t)n * ra.ninj;
             float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            for (int e = g.e0; e < g.e1; e++) {
-                const InjEntry en = a.ent[e];
+            for (int e = g.e0 - ebase; e < g.e1 - ebase; e++) {
+                const InjEntry en = ecache[e];
                 const int dz = en.jz - 4 * g.col;
-                const float v = a.inj_scale * en.w * val[en.id];
+                const float v = a.inj_scale * en.w * vbuf[buf * RS_MAXE + e];
 #pragma unroll
                 for (int q = 0; q < 4; q++)
                     if (q == dz) acc[q] += v;
             }
-            staged[buf * (RS_MAXG + 1) + tid] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            staged[tid] = make_float4(acc[0], acc[1], acc[2], acc[3]);
         }
     };
-    stage(ra.n0, 0);
+    fetch_values(ra.n0, 0);
+    cp_async_wait<0>();
     __syncthreads();
 
     for (int s = 0; s < ra.nsteps; s++) {
@@ -247,6 +268,9 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
         const unsigned ep = ra.ep0 + (unsigned)s + 1u;
         float *xb = ra.xbuf + ((size_t)(ep & 1u) * ra.NB + b) * (size_t)(8 * nq4);
         RS_STAMP(0);
+        stage(s & 1);                                      // this step's amounts (values fetched during the previous step)
+        if (s + 1 < ra.nsteps) fetch_values(n + ra.dir, (s + 1) & 1);
+        __syncthreads();
         if (!comm) {
             // ---- sweep: boundary rows first, then towards the middle ----------------------------------------------
             {
@@ -262,15 +286,19 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
                 float4 q[9];                                            // stream rows i-4 .. i+4
 #pragma unroll
                 for (int i = 0; i < 8; i++) q[i] = (nrow_t > 0 ? ld4(up + (i - 4) * rs) : make_float4(0.f, 0.f, 0.f, 0.f));
-                float4 k24 = nrow_t > 0 ? ldg4(K2p) : make_float4(0.f, 0.f, 0.f, 0.f), k24n = nrow_t > 1 ? ldg4(K2p + ksx) : k24;
+                const float *ksp = Ks + rstart * nq4 + jz;              // CL: K2 of the current row in shared memory
+                float4 k24 = make_float4(0.f, 0.f, 0.f, 0.f), k24n = k24;
+                if (!CL) { k24 = nrow_t > 0 ? ldg4(K2p) : k24; k24n = nrow_t > 1 ? ldg4(K2p + ksx) : k24; }
                 auto row = [&](int i, bool publish) {
                     q[8] = ld4(up + rs4);
                     const float4 c = q[4];
                     const float4 zm = ld4(up - 4), zp = ld4(up + 4);
                     const float4 du4 = ld4(dp);
-                    const float4 k2c = k24;
-                    k24 = k24n;
-                    if (i + 2 < nrow_t) k24n = ldg4(kp);   // K2 (L2) two rows ahead of its use
+                    const float4 k2c = CL ? ld4(ksp) : k24;
+                    if (!CL) {
+                        k24 = k24n;
+                        if (i + 2 < nrow_t) k24n = ldg4(kp);   // K2 (L2) two rows ahead of its use
+                    }
                     const float sxc = s_dx[rr], k1xc = s_k1x[rr];
                     const float win[12] = {zm.x, zm.y, zm.z, zm.w, c.x, c.y, c.z, c.w, zp.x, zp.y, zp.z, zp.w};
                     const float cc[4] = {c.x, c.y, c.z, c.w};
@@ -311,7 +339,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
                         dhi = fma2(pk(k1[2], k1[3]), duhi, mul2(k2hi, lhi));
                     }
                     if (im & 1u) {   // a3: K2 * scale * w * val
-                        const float4 iv = staged[(s & 1) * (RS_MAXG + 1) + gmap[rr * nq + col] - 1];
+                        const float4 iv = staged[gmap[rr * nq + col] - 1];
                         dlo = fma2(k2lo, pk(iv.x, iv.y), dlo);
                         dhi = fma2(k2hi, pk(iv.z, iv.w), dhi);
                     }
@@ -342,7 +370,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
                             if (rr >= R - 4) __stcg(reinterpret_cast<float4 *>(xb + (4 + rr - (R - 4)) * nq4 + jz), un);
                         }
                     }
-                    up += rs; unp += rs; dp += dstep; kp += ksx; hp += hstep; rr += dirn;
+                    up += rs; unp += rs; dp += dstep; kp += ksx; ksp += dstep; hp += hstep; rr += dirn;
 #pragma unroll
                     for (int k = 0; k < 8; k++) q[k] = q[k + 1];
                 };
@@ -359,7 +387,6 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
                 for (int i = nbnd; i < nrow_t; i++) row(i, false);
             }
             RS_STAMP(1);
-            if (s + 1 < ra.nsteps) stage(n + ra.dir, (s + 1) & 1);     // next step's injection amounts: off the critical path
         } else {
             // ---- communication warp ---------------------------------------------------------------------------------
             asm volatile("bar.sync 1, %0;" ::"n"(RS_THREADS) : "memory");      // every boundary row of the slab is published
@@ -385,6 +412,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) acoustic2d_resident_kernel(cons
             }
             RS_STAMP(2);
         }
+        cp_async_wait<0>();                                    // this thread's share of the next step's values has landed
         if (CL) {
             // every block of the cluster has written its rows (and its neighbours' halo rows): release / acquire at cluster scope
             asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");

@@ -612,10 +612,13 @@ static int build_geometry(rtm_ctx *c, int slot, int ninj, const float *inj_xyz, 
         per_slab[m].assign(std::max(1, c->res[m].nb), 0);
         if (!g->res_ok[m]) continue;
         long long lrow = -1; int lq = -1;
+        std::vector<int> ents(per_slab[m].size(), 0);
         for (const Tmp &t : tmp) {
-            if (t.row != lrow || (t.jz >> 2) != lq) { per_slab[m][slab_of_row(c, c->res[m].nb, (int)t.row)]++; lrow = t.row; lq = t.jz >> 2; }
+            const int sl = slab_of_row(c, c->res[m].nb, (int)t.row);
+            ents[sl]++;
+            if (t.row != lrow || (t.jz >> 2) != lq) { per_slab[m][sl]++; lrow = t.row; lq = t.jz >> 2; }
         }
-        for (int v : per_slab[m]) g->res_ok[m] = g->res_ok[m] && v <= RS_MAXG;
+        for (size_t i = 0; i < ents.size(); i++) g->res_ok[m] = g->res_ok[m] && per_slab[m][i] <= RS_MAXG && ents[i] <= RS_MAXE;
         std::fill(per_slab[m].begin(), per_slab[m].end(), 0);
     }
     for (int s = 0; s < nsmp; s++) {
@@ -676,9 +679,10 @@ static int make_tmaps(rtm_ctx *c) {
 }
 
 // ---- resident 2D kernel: plan and launch (acoustic2d_resident.cuh) ----------------------------------------------------
-static size_t resident_smem(const Layout &L, int rmax) {
+static size_t resident_smem(const Layout &L, int rmax, int mode) {
     const int nq = (L.Pz + 3) / 4, spz = nq * 4 + 8;
-    return (size_t)2 * (rmax + 8) * spz * 4 + (size_t)rmax * nq * 16 + (size_t)(RS_MAXG + 1) * (2 * 16 + sizeof(RsGroup)) +
+    return (size_t)2 * (rmax + 8) * spz * 4 + (size_t)rmax * nq * 16 * (mode == 0 ? 2 : 1) /* du (+ K2 in the cluster mode) */ +
+           (size_t)(RS_MAXG + 1) * (16 + sizeof(RsGroup)) + (size_t)RS_MAXE * (sizeof(InjEntry) + 8) +
            (size_t)RS_MAXS * sizeof(RsSample) + (size_t)rmax * nq + 16;
 }
 // Mode 1 (exchange through L2): one slab per SM, the largest NB <= #SM whose slabs have >= 4 rows (a halo comes from ONE
@@ -699,7 +703,7 @@ static int plan_resident(rtm_ctx *c) {
             if (m == 1 ? 2 * nq > RS_THREADS - 32 : nq > RS_THREADS) break;   // mode 1: two sweeping threads per column + the communication warp
             const int rmax = (L.Px + nb - 1) / nb;
             if (rmax > RS_MAXROWS) break;
-            const size_t smem = resident_smem(L, rmax);
+            const size_t smem = resident_smem(L, rmax, m);
             if (smem + 1024 > (size_t)smem_max) break;
             CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             if (m == 0) {
