@@ -386,6 +386,13 @@ __device__ __forceinline__ void inject_quad(const StepArgs &a, long long row, in
 // later groups are issued before the stores of the current one; see flush_role).
 // Measured (per-step fused schedule): 2D acoustic 68.5 us at DEPTH 1 / 4 blocks per SM against 72.9 us at DEPTH 2 /
 // 3 blocks; TTI 246 us against 218 us: the kernels pick their own depth.
+// Per-step fused probing: ask L2 for this thread's 16 bytes of every probe plane at the START of the step kernel, so that
+// the DRAM reads of the planes are spread over the stencil phase instead of starting behind it (the planes are written
+// by the previous launch; L2 is the coherence point, so the request may even precede griddepcontrol.wait).
+__device__ __forceinline__ void prefetch_planes(const float *p, long long Nu, int r) {
+    for (int k = 0; k < r; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(p + (long long)k * Nu));
+}
+
 template <int DEPTH>
 __device__ __forceinline__ void probe_quad(float *p, long long Nu, const float *__restrict__ Zrow, int r, float4 v) {
     constexpr int G = 4;
