@@ -163,6 +163,9 @@ __global__ void __launch_bounds__(256, 2) acoustic3d_stream_kernel(const __grid_
     float *ph = a.hist + (((long long)(x0 - L.nb) * L.ny + iy) * L.upz + iz);   // dereferenced inside the physical grid only
 
     const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    // (Unrolling the plane loop by 8 with a circular queue of 8 register quads removes the 32 moves per plane that slide
+    // this queue and makes every ring offset a constant, but the body grows 8-fold (142 KB of SASS) and the launch gets
+    // slower: c4 0.749 ms per step against 0.677.  Kept rolled.)
     float4 q[9];   // planes p-4 .. p+4 of this thread's quad; q[8] is filled from the ring at the top of iteration p
 #pragma unroll
     for (int i = 0; i < 8; i++) q[i] = ld_c ? ld4(pc + (i - 4) * sx) : zero4;
