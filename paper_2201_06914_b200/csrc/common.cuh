@@ -263,17 +263,25 @@ __device__ __forceinline__ void flush_role(const StepArgs &a, float *sz, int tid
                     const int kn = k + G * DEPTH + i;
                     ring[s][i] = (kn < r) ? ldcs2(p + (long long)kn * a.pNu) : make_float2(0.f, 0.f);
                 }
+                // one FFMA2 per (plane, history slot): both x lanes of the float2 in one issue slot, each lane rounded
+                // exactly like the scalar FMA it replaces
+                f32x2 ap[G];
+#pragma unroll
+                for (int i = 0; i < G; i++) ap[i] = pk(acc[i].x, acc[i].y);
 #pragma unroll
                 for (int j = 0; j < TM; j++) {
                     const float4 z = ld4(sz + j * zr + k);
-                    acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
-                    acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
-                    acc[2].x = fmaf(z.z, h[j].x, acc[2].x); acc[2].y = fmaf(z.z, h[j].y, acc[2].y);
-                    acc[3].x = fmaf(z.w, h[j].x, acc[3].x); acc[3].y = fmaf(z.w, h[j].y, acc[3].y);
+                    const f32x2 hp = pk(h[j].x, h[j].y);
+                    ap[0] = fma2(pk(z.x, z.x), hp, ap[0]);
+                    ap[1] = fma2(pk(z.y, z.y), hp, ap[1]);
+                    ap[2] = fma2(pk(z.z, z.z), hp, ap[2]);
+                    ap[3] = fma2(pk(z.w, z.w), hp, ap[3]);
                 }
 #pragma unroll
-                for (int i = 0; i < G; i++)
+                for (int i = 0; i < G; i++) {
+                    upk(ap[i], acc[i].x, acc[i].y);
                     if (k + i < r) stcs2(p + (long long)(k + i) * a.pNu, acc[i]);
+                }
             }
         }
     }
@@ -328,17 +336,22 @@ __device__ __forceinline__ void flush_role4(const StepArgs &a, float *sz, int ti
                     const int kn = k + G * DEPTH + i;
                     ring[s][i] = (kn < r) ? ldcs4(p + (long long)kn * a.pNu) : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
+                f32x2 alo[G], ahi[G];   // packed FMAs, see flush_role
+#pragma unroll
+                for (int i = 0; i < G; i++) { alo[i] = pk(acc[i].x, acc[i].y); ahi[i] = pk(acc[i].z, acc[i].w); }
 #pragma unroll
                 for (int j = 0; j < TM; j++) {
                     const float2 z = *reinterpret_cast<const float2 *>(sz + j * zr + k);
-                    acc[0].x = fmaf(z.x, h[j].x, acc[0].x); acc[0].y = fmaf(z.x, h[j].y, acc[0].y);
-                    acc[0].z = fmaf(z.x, h[j].z, acc[0].z); acc[0].w = fmaf(z.x, h[j].w, acc[0].w);
-                    acc[1].x = fmaf(z.y, h[j].x, acc[1].x); acc[1].y = fmaf(z.y, h[j].y, acc[1].y);
-                    acc[1].z = fmaf(z.y, h[j].z, acc[1].z); acc[1].w = fmaf(z.y, h[j].w, acc[1].w);
+                    const f32x2 hlo = pk(h[j].x, h[j].y), hhi = pk(h[j].z, h[j].w);
+                    const f32x2 z0 = pk(z.x, z.x), z1 = pk(z.y, z.y);
+                    alo[0] = fma2(z0, hlo, alo[0]); ahi[0] = fma2(z0, hhi, ahi[0]);
+                    alo[1] = fma2(z1, hlo, alo[1]); ahi[1] = fma2(z1, hhi, ahi[1]);
                 }
 #pragma unroll
-                for (int i = 0; i < G; i++)
+                for (int i = 0; i < G; i++) {
+                    upk(alo[i], acc[i].x, acc[i].y); upk(ahi[i], acc[i].z, acc[i].w);
                     if (k + i < r) stcs4(p + (long long)(k + i) * a.pNu, acc[i]);
+                }
             }
         }
     }
