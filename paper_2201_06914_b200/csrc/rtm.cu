@@ -355,32 +355,38 @@ static int coeffs_host_impl(const rtm_config *cfg, const float *h_vp, const floa
         }
         tab += P[a];
     }
+    // Edge replication into the layer as per-axis index maps (physical index of every padded index), then one sweep over
+    // the padded grid in canonical order.  sigma dt = (x part + y part) + z part, in that association: it is rounded
+    // once to fp32 through K2 and must give the same bits on every implementation of O1.
+    std::vector<int> src_of[3];
     const int nn[3] = {L.nx, L.ny, L.nz};
-    for (int jx = 0; jx < L.Px; jx++)
-        for (int jy = 0; jy < L.Py; jy++)
-            for (int jz = 0; jz < L.Pzc; jz++) {
-                const int ix = std::min(std::max(jx - lay[0], 0), nn[0] - 1);
-                const int iy = std::min(std::max(jy - lay[1], 0), nn[1] - 1);
-                const int iz = std::min(std::max(jz - lay[2], 0), nn[2] - 1);
-                const long long s = ((long long)ix * L.ny + iy) * L.nz + iz;
-                const long long d = ((long long)jx * L.Py + jy) * L.Pzc + jz;
+    for (int a = 0; a < 3; a++) {
+        src_of[a].resize(P[a]);
+        for (int j = 0; j < P[a]; j++) src_of[a][j] = std::min(std::max(j - lay[a], 0), nn[a] - 1);
+    }
+    long long d = 0;
+    for (int jx = 0; jx < L.Px; jx++) {
+        const long long sx_ = (long long)src_of[0][jx] * L.ny;
+        for (int jy = 0; jy < L.Py; jy++) {
+            const long long sxy = (sx_ + src_of[1][jy]) * L.nz;
+            const double pxy = prof[0][jx] + prof[1][jy];
+            for (int jz = 0; jz < L.Pzc; jz++, d++) {
+                const long long s = sxy + src_of[2][jz];
                 const double c = h_vp[s];
-                const double sdt = prof[0][jx] + prof[1][jy] + prof[2][jz];
-                h_K2[d] = (float)(c * c * dt * dt / (h * h * (1.0 + sdt)));
-                if (tti) {
-                    const double e = h_eps[s];
-                    const double dl = std::min((double)h_delta[s], e);
-                    const double th = h_theta[s];
-                    h_epsh[d] = (float)(1.0 + 2.0 * e);
-                    h_delh[d] = (float)std::sqrt(1.0 + 2.0 * dl);
-                    h_cos[d] = (float)std::cos(th);
-                    h_sin[d] = (float)std::sin(th);
-                    if (h_phi) {
-                        h_cosp[d] = (float)std::cos((double)h_phi[s]);
-                        h_sinp[d] = (float)std::sin((double)h_phi[s]);
-                    }
+                h_K2[d] = (float)(c * c * dt * dt / (h * h * (1.0 + (pxy + prof[2][jz]))));
+                if (!tti) continue;
+                const double e = h_eps[s];
+                h_epsh[d] = (float)(1.0 + 2.0 * e);
+                h_delh[d] = (float)std::sqrt(1.0 + 2.0 * std::min((double)h_delta[s], e));
+                h_cos[d] = (float)std::cos((double)h_theta[s]);
+                h_sin[d] = (float)std::sin((double)h_theta[s]);
+                if (h_phi) {
+                    h_cosp[d] = (float)std::cos((double)h_phi[s]);
+                    h_sinp[d] = (float)std::sin((double)h_phi[s]);
                 }
             }
+        }
+    }
     return RTM_OK;
 }
 extern "C" int rtm_coeffs_host(const rtm_config *cfg, const float *h_vp, const float *h_eps, const float *h_delta,
