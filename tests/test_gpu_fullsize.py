@@ -118,3 +118,23 @@ def test_3d_streaming_kernel_many_tiles_against_oracle():
             for sy in (slice(0, 12), slice(12, 24)):
                 for sz in (slice(0, 130), slice(130, 260)):
                     assert np.abs(img[sx, sy, sz]).max() > 0
+
+
+def test_c4_full_grid_compressed_wavefields_and_image_against_oracle():
+    """The full 512 x 512 x 256 (+40) grid in the launch configuration bench.py times (T = 32, TMA streaming kernel:
+    74 y-tiles, 3 z-tiles, 19 x-chunks), 12 + 12 steps with r = 2 probes (so that the oracle's fp64 planes stay at 1 GB
+    each): receiver data, Uz, Vz, image and a 3-offset gather against the oracle, element by element."""
+    p = ri.make_c4()
+    nt = 12
+    p.nt, p.r = nt, 2
+    p.wav, p.Z = np.ascontiguousarray(p.wav[:nt]), np.ascontiguousarray(p.Z[:nt, :2])
+    offs = np.array([-2, 0, 3], np.int32)
+    g = run_gpu(p, offsets=offs, probe_block=32, want_qadj=False)
+    o = run_oracle(p, g["din"], offsets=offs)
+    for k in ("data", "Uz", "Vz", "image", "gather"):
+        tol = TOL_FIELD if k == "data" else TOL_IMAGE
+        e = rel(g[k], o[k])
+        print("c4 full grid nt=12 r=2", k, "%.2e" % e)
+        assert e <= tol, (k, e)
+        elem_ok(g[k], o[k], tol, k)
+    assert np.abs(o["image"]).max() > 0

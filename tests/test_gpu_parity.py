@@ -247,6 +247,15 @@ def test_resident_kernel_is_bit_identical_to_the_streaming_kernel(n, nb, T, mode
         assert np.array_equal(a[k], b[k]), k
 
 
+def test_dense_geometry_falls_back_from_the_resident_kernel():
+    """More receivers per slab than the resident kernel's per-slab tables hold (256 sampled points, 255 injection groups,
+    256 entries): the pass must take the streaming kernel (as many launches as steps) and still match the oracle; the
+    forward pass of the same context with its two sources stays resident."""
+    p = ri.random_acoustic(2, n=(70, 61), nb=8, nt=40, r=4, seed=31, nsrc=2, nrec=6000)
+    g, o, e = check_all(p, offsets=np.array([-1, 0, 2], np.int32), probe_block=16)
+    assert g["launches"] > 2 * p.nt          # forward sampling of 6000 receivers and their injection: one launch per step
+
+
 def test_time_block_of_32_steps():
     p2 = ri.random_acoustic(2, n=(70, 61), nb=8, nt=83, r=6, seed=31, nsrc=2, nrec=5)
     check_all(p2, snap_steps=[40, 82], offsets=np.array([-2, 0, 1], np.int32), probe_block=32)
