@@ -34,6 +34,18 @@ static thread_local char g_cuda_err[256] = "";
 
 static inline long long rup(long long v, long long m) { return (v + m - 1) / m * m; }
 
+// Opt a kernel in to the largest dynamic shared memory the device allows (its static shared memory counts against the
+// same limit).  The attribute belongs to the function on a device and is shared by all contexts and threads, which is why
+// it is never set to one context's own need.
+static cudaError_t optin_max_smem(const void *fn, int device) {
+    int smem_max = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    if (e != cudaSuccess) return e;
+    cudaFuncAttributes fa;
+    if ((e = cudaFuncGetAttributes(&fa, fn)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - (int)fa.sharedSizeBytes);
+}
+
 // Every entry point runs on the device that owns the context's workspace, whatever device is current in the calling
 // thread; the previous device is restored on return.
 struct DeviceGuard {
@@ -711,7 +723,9 @@ static int plan_resident(rtm_ctx *c) {
             if (rmax > RS_MAXROWS) break;
             const size_t smem = resident_smem(L, rmax, m);
             if (smem + 1024 > (size_t)smem_max) break;
-            CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            // the opt-in is a property of the FUNCTION on this device, shared by every context: always the device maximum,
+            // never this context's own need (a second, smaller context must not lower it under the first one's feet)
+            CU(optin_max_smem(fn, c->device));
             if (m == 0) {
                 CU(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
                 cudaLaunchAttribute at[1];
@@ -864,16 +878,17 @@ static int launch_ex(rtm_ctx *c, K kernel, const StepArgs &a, unsigned nblocks, 
     memset(&lc, 0, sizeof lc);
     lc.gridDim = dim3(nblocks, 1, 1); lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
     lc.attrs = at; lc.numAttrs = 1;
-    if (smem > 48 * 1024) {   // opt in to large dynamic shared memory, once per kernel and size
-        // (the attribute is per device: the cache is keyed by it)
-        struct Done { int dev; const void *fp; size_t smem; };
+    if (smem > 48 * 1024) {
+        // opt in to large dynamic shared memory, once per (device, kernel) and thread: the attribute belongs to the
+        // function on a device and is shared by all contexts and threads, so it is always set to the device maximum
+        struct Done { int dev; const void *fp; };
         static thread_local std::vector<Done> done;
         const void *fp = (const void *)kernel;
         bool ok = false;
-        for (auto &d : done) ok = ok || (d.dev == c->device && d.fp == fp && d.smem >= smem);
+        for (auto &d : done) ok = ok || (d.dev == c->device && d.fp == fp);
         if (!ok) {
-            CU(cudaFuncSetAttribute(fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            done.push_back({c->device, fp, smem});
+            CU(optin_max_smem(fp, c->device));
+            done.push_back({c->device, fp});
         }
     }
     CU(cudaLaunchKernelEx(&lc, kernel, a));

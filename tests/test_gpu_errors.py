@@ -134,3 +134,32 @@ def test_no_kernel_writes_outside_the_workspace_or_its_outputs(T):
             assert torch.isnan(buf[:G]).all() and torch.isnan(buf[-G:]).all()
             assert torch.isfinite(view).all()
         m.close()
+
+
+def test_contexts_of_different_sizes_coexist():
+    """The large-shared-memory opt-in belongs to a kernel function on a device, not to a context: a second, smaller
+    context (2D resident kernel with a small slab, 3D streaming kernel) must not break the launches of a larger one that
+    is still alive, whatever the order in which they are created and used."""
+    import torch
+    from paper_2201_06914_b200 import Rtm
+    big = ri.random_acoustic(2, n=(300, 520), nb=20, nt=60, r=4, seed=3, nrec=40)       # resident: slabs of ~21 rows x 560 points
+    small = ri.random_acoustic(2, n=(40, 36), nb=8, nt=60, r=4, seed=4)
+    vol = ri.random_acoustic(3, n=(24, 20, 28), nb=4, nt=40, r=4, seed=5)
+    ms = []
+    for p in (big, small, vol):
+        m = Rtm.from_problem(p, probe_block=8)
+        m.set_model_from_earth(p.vp)
+        m.set_probes(p.Z)
+        ms.append((m, p))
+    outs = {}
+    for rnd in range(2):
+        for i in (0, 1, 2, 1, 0):
+            m, p = ms[i]
+            d = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz).cpu().numpy()
+            assert np.isfinite(d).all() and np.abs(d).max() > 0
+            if i in outs:
+                assert np.array_equal(outs[i], d)
+            outs[i] = d
+    torch.cuda.synchronize()
+    for m, _ in ms:
+        m.close()
