@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(256) gather_xy_kernel(Layout L, const float *_
 constexpr int GT_X = 32, GT_HP = 48;
 __host__ __device__ constexpr int gt_rows(int hp) { return GT_X + hp - 1; }
 __host__ __device__ constexpr int gt_threads(int hp) { return 32 * (GT_X / 8) * (hp / 8); }
-__host__ __device__ constexpr int gt_stages(int hp) { return hp <= 16 ? 4 : 2; }   // probes in flight (shared-memory buffers)
+__host__ __device__ constexpr int gt_stages(int hp) { return 4; }   // probes in flight (shared-memory buffers)
 __host__ __device__ constexpr int gt_smem(int hp) { return gt_stages(hp) * 2 * gt_rows(hp) * 32 * 4; }
 
 template <int HP, bool XY>

@@ -1193,6 +1193,7 @@ extern "C" int rtm_offset_gather(rtm_ctx *c, int nh, const int *h_offsets, float
     for (int i = 1; i < nh && run; i++) run = h_offsets[i] == h_offsets[i - 1] + 1;
     if (run) {
         const dim3 grid((unsigned)(((long long)L.ny * L.upz) / 32), (unsigned)((L.nx + GT_X - 1) / GT_X), 1);
+        if (nh > 16) CU(optin_max_smem((const void *)gather_tiled_kernel<GT_HP, false>, c->device));   // 81 KB of staging: 4 probes in flight
         if (nh <= 16) gather_tiled_kernel<16, false><<<grid, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], nullptr, 0, scale, d_gather);
         else gather_tiled_kernel<GT_HP, false><<<grid, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, nh, h_offsets[0], nullptr, 0, scale, d_gather);
     } else {
@@ -1246,8 +1247,10 @@ extern "C" int rtm_offset_gather_xy(rtm_ctx *c, int nh, const int *h_offsets_xy,
         const int4 *d_runs = (const int4 *)(c->offs + (3 + cls) * 4096);
         if (cls == 0)
             gather_tiled_kernel<16, true><<<(unsigned)nblk, gt_threads(16), gt_smem(16), st>>>(L, c->Uz, c->Vz, c->rp, 0, 0, d_runs, nrun[cls], scale, d_gather);
-        else
+        else {
+            CU(optin_max_smem((const void *)gather_tiled_kernel<GT_HP, true>, c->device));
             gather_tiled_kernel<GT_HP, true><<<(unsigned)nblk, gt_threads(GT_HP), gt_smem(GT_HP), st>>>(L, c->Uz, c->Vz, c->rp, 0, 0, d_runs, nrun[cls], scale, d_gather);
+        }
         c->launches++;
     }
     if (nl) {
