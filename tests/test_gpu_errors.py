@@ -163,3 +163,22 @@ def test_contexts_of_different_sizes_coexist():
     torch.cuda.synchronize()
     for m, _ in ms:
         m.close()
+
+
+def test_option_values_are_validated():
+    """rx = 32 used to be stored unchecked and left half of the rows un-updated; only the kernel's
+    instances are accepted now, and unknown options / values return RTM_EINVAL."""
+    from paper_2201_06914_b200 import RTMError
+    p = ri.random_acoustic(2, n=(30, 28), nb=4, nt=10, r=2)
+    m = _mk(p, probe_block=8)
+    for name, bad in (("rx", 32), ("rx", 3), ("rx", -1), ("resident", 4), ("resident", -1), ("no_such_option", 1), ("dbg", 1)):
+        with pytest.raises(RTMError) as e:
+            m.set_option(name, bad)
+        assert e.value.code == -1, (name, bad)
+    for name, ok in (("rx", 16), ("rx", 0), ("resident", 0), ("resident", 3), ("pdl", 0), ("time_steps", 1)):
+        m.set_option(name, ok)
+    m.close()
+    m3 = _mk(ri.random_acoustic(3, n=(14, 12, 10), nb=4, nt=5, r=2), probe_block=8)
+    with pytest.raises(RTMError):
+        m3.set_option("rx", 4)                      # the 2D streaming kernel's knob
+    m3.close()
