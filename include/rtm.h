@@ -210,6 +210,33 @@ float rtm_pass_ms_mean(rtm_ctx *ctx, int which, int count);
  * -DRTM_DEBUG (see the end of this header); the product build has neither.                                */
 int rtm_set_option(rtm_ctx *ctx, const char *name, int value);
 
+/* ---- the one entry point that allocates nothing ------------------------------------------------------------------
+ * Offset gather (Eq. 4; reading C11) of caller-held compressed wavefields, for callers that cannot
+ * allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): no context, no
+ * workspace, no cudaMalloc / cudaFree / cudaMallocHost / event creation, no memcpy -- two kernel launches on `cuda_stream`
+ * of the thread's CURRENT device and nothing else.
+ *   gather[ih][x][z] = scale * sum_k U[k][x + h][z] V[k][x - h][z],  h = h_offsets[ih] grid points along x, zero where
+ *   x + h or x - h leaves [0, nx);  h = 0 is Eq. 3's image.  2D grids.
+ *   d_U, d_V   [r][nx][nz] fp32, DEVICE (the layout rtm_export_probes writes); read only
+ *   h_offsets  [nh] HOST ints (passed to the device as a kernel argument: they may be reused when the call returns)
+ *   d_gather   [nh][nx][nz] fp32, DEVICE, caller-owned; every element is written
+ * Same arithmetic as rtm_offset_gather's generic kernel (the same gather_kernel: one fma per probe, k ascending), so
+ * the two agree bit for bit on the same Uz / Vz.
+ * Scratch: the kernel's operands -- U and V re-pitched to rows of 4 ceil(nz / 4) floats (16-byte loads) and the
+ * offsets table -- live in ONE file-scope `static __device__` array of RTM_STATIC_SCRATCH_BYTES, which every GPU that
+ * loads the library holds until the process exits.  Requests with
+ *   256 + 2 * r * nx * 4 ceil(nz / 4) * 4 bytes > RTM_STATIC_SCRATCH_BYTES   or   nh > RTM_STATIC_MAX_OFFSETS
+ * are rejected with RTM_ELIMIT before anything is launched.  Every call, on every stream and from every thread, shares
+ * the array: it keeps the previous call's contents (each call rewrites all of what it reads, pad columns as zeros, so
+ * nothing needs clearing by the caller), and two calls that overlap on the GPU (different streams without an ordering
+ * between them) RACE on it.  Calls on one stream are ordered by the stream.
+ * Errors: RTM_EINVAL (NULL, nx / nz / r / nh < 1, |h| >= nx), RTM_ELIMIT, RTM_ECUDA.                              */
+#define RTM_STATIC_SCRATCH_BYTES (16u << 20)
+#define RTM_STATIC_MAX_OFFSETS 64
+#define RTM_ELIMIT (-5) /* size beyond the static scratch: RTM_STATIC_SCRATCH_BYTES / RTM_STATIC_MAX_OFFSETS */
+int rtm_offset_gather_static(int nx, int nz, int r, const float *d_U, const float *d_V, int nh, const int *h_offsets,
+                             float scale, float *d_gather, void *cuda_stream);
+
 const char *rtm_strerror(int code);
 const char *rtm_last_cuda_error(void);
 

@@ -2,5 +2,5 @@
 imaging condition fused into the time loop.  Thin Python binding over the C ABI in include/rtm.h.
 
 There is no CPU fallback: importing the binding fails loudly if the CUDA library is missing."""
-from .binding import (RTMError, Rtm, RtmConfig, coeffs_host, coeffs_host3, lib_path, load_library, probes_dtt_host, probes_qr_host,
+from .binding import (RTMError, Rtm, RtmConfig, coeffs_host, coeffs_host3, lib_path, load_library, offset_gather_static, probes_dtt_host, probes_qr_host,
                       workspace_bytes)  # noqa: F401

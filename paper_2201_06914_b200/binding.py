@@ -14,7 +14,7 @@ _lib = None
 
 EXPORTS = ["rtm_workspace_bytes", "rtm_create", "rtm_destroy", "rtm_coeffs_host", "rtm_coeffs_host3", "rtm_set_model", "rtm_set_model3",
            "rtm_set_probes", "rtm_probes_dtt_host", "rtm_probes_qr_host", "rtm_forward_probe", "rtm_adjoint_image", "rtm_image", "rtm_offset_gather",
-           "rtm_offset_gather_xy",
+           "rtm_offset_gather_xy", "rtm_offset_gather_static",
            "rtm_shot_staging_bytes", "rtm_shot_host", "rtm_export_probes", "rtm_set_snapshots",
            "rtm_export_coeff", "rtm_last_pass_ms", "rtm_pass_ms_mean", "rtm_launch_count", "rtm_set_option", "rtm_strerror", "rtm_last_cuda_error"]
 
@@ -63,6 +63,7 @@ def load_library():
     lib.rtm_image.argtypes = [vp, fp, ip, vp, vp]
     lib.rtm_offset_gather.argtypes = [vp, ip, vp, fp, vp, vp]
     lib.rtm_offset_gather_xy.argtypes = [vp, ip, vp, fp, vp, vp]
+    lib.rtm_offset_gather_static.argtypes = [ip, ip, ip, vp, vp, ip, vp, fp, vp, vp]
     lib.rtm_shot_staging_bytes.restype = C.c_size_t
     lib.rtm_shot_staging_bytes.argtypes = [cfgp, ip, ip, ip]
     lib.rtm_shot_host.argtypes = [vp, ip, vp, vp, ip, vp, vp, vp, fp, vp, ip, vp, vp, vp, C.c_size_t, vp]
@@ -167,6 +168,28 @@ def probes_dtt_host(Z, dt):
     Z = np.ascontiguousarray(Z, np.float32)
     out = np.empty_like(Z)
     _check(load_library().rtm_probes_dtt_host(Z.shape[0], Z.shape[1], float(dt), _hp(Z), _hp(out)))
+    return out
+
+
+STATIC_SCRATCH_BYTES = 16 << 20     # rtm.h: RTM_STATIC_SCRATCH_BYTES
+STATIC_MAX_OFFSETS = 64             # rtm.h: RTM_STATIC_MAX_OFFSETS
+
+
+def offset_gather_static(U, V, offsets, scale, out, stream=None):
+    """rtm_offset_gather_static: the entry point that allocates nothing.  U, V: CUDA fp32 tensors [r][nx][nz] on the
+    current device; out: caller-allocated CUDA fp32 tensor [nh][nx][nz] (this wrapper allocates nothing on the device
+    either); offsets: host ints.  Calls share one static device array: keep them ordered on the GPU."""
+    import torch
+    offs = np.ascontiguousarray(offsets, np.int32)
+    r, nx, nz = (int(x) for x in U.shape)
+    for x in (U, V, out):
+        if not (x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()):
+            raise ValueError("offset_gather_static takes contiguous fp32 CUDA tensors")
+    if tuple(V.shape) != (r, nx, nz) or tuple(out.shape) != (len(offs), nx, nz):
+        raise ValueError("offset_gather_static: V must be [r][nx][nz], out [nh][nx][nz]")
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _check(load_library().rtm_offset_gather_static(nx, nz, r, C.c_void_p(U.data_ptr()), C.c_void_p(V.data_ptr()), len(offs),
+                                                   _hp(offs), float(scale), C.c_void_p(out.data_ptr()), C.c_void_p(st)))
     return out
 
 

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1403,6 +1404,78 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     return RTM_EINVAL;
 }
 
+// ---- the entry point that allocates nothing (rtm.h: rtm_offset_gather_static) --------------------------------------
+// The operands of gather_kernel (image.cuh) -- U and V in rows of upz floats, the offsets table -- are workspace memory in
+// a context; here they live in a file-scope device array, so the call needs no context and no allocation.  In host code
+// the NAME g_static_scratch is only a stand-in for the symbol (not a device address): the address comes from
+// cudaGetSymbolAddress, once per device, with that device current, and is what the kernels are given.
+static __device__ __align__(256) float g_static_scratch[RTM_STATIC_SCRATCH_BYTES / 4];
+static std::mutex g_static_mu;
+static float *g_static_ptr[64];   // device address of g_static_scratch, per device ordinal
+
+struct StaticOffsets { int h[RTM_STATIC_MAX_OFFSETS]; };
+
+// [planes][nx][nz] of U and of V -> rows of upz floats in the scratch (pad columns are WRITTEN as zeros: the array keeps
+// the previous call's contents); the first nh threads also store the offsets table, which arrives as a kernel argument
+__global__ void __launch_bounds__(256) static_pack_kernel(int nz, int upz, long long rows, const float *__restrict__ U,
+                                                          const float *__restrict__ V, float *__restrict__ sU,
+                                                          float *__restrict__ sV, int *__restrict__ sOffs, int nh,
+                                                          const __grid_constant__ StaticOffsets offs) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < nh) sOffs[t] = offs.h[t];
+    if (t >= rows * upz) return;
+    const int iz = (int)(t % upz);
+    const long long row = t / upz;
+    const bool in = iz < nz;
+    sU[t] = in ? U[row * nz + iz] : 0.0f;
+    sV[t] = in ? V[row * nz + iz] : 0.0f;
+}
+
+static int static_scratch_address(float **out) {
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return RTM_EINVAL;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_scratch));
+        g_static_ptr[dev] = (float *)p;
+    }
+    *out = g_static_ptr[dev];
+    return RTM_OK;
+}
+
+extern "C" int rtm_offset_gather_static(int nx, int nz, int r, const float *d_U, const float *d_V, int nh, const int *h_offsets,
+                                        float scale, float *d_gather, void *stream) {
+    if (nx < 1 || nz < 1 || r < 1 || nh < 1 || !d_U || !d_V || !h_offsets || !d_gather) return RTM_EINVAL;
+    if (nh > RTM_STATIC_MAX_OFFSETS) return RTM_ELIMIT;
+    const long long cap = (long long)(RTM_STATIC_SCRATCH_BYTES / 4) - 64;   // floats after the offsets table (256 B)
+    const long long upz = rup(nz, 4);
+    if (upz > cap || nx > cap / upz || r > cap / (2 * upz * nx)) return RTM_ELIMIT;
+    StaticOffsets offs;
+    for (int i = 0; i < nh; i++) {
+        if (std::abs((long long)h_offsets[i]) >= nx) return RTM_EINVAL;
+        offs.h[i] = h_offsets[i];
+    }
+    for (int i = nh; i < RTM_STATIC_MAX_OFFSETS; i++) offs.h[i] = 0;
+    float *scratch = nullptr;
+    int rc = static_scratch_address(&scratch);
+    if (rc) return rc;
+    int *sOffs = reinterpret_cast<int *>(scratch);
+    float *sU = scratch + 64, *sV = sU + (long long)r * nx * upz;
+    Layout L{};
+    L.nd = 2; L.nx = nx; L.ny = 1; L.nz = nz;
+    L.upz = (int)upz;
+    L.Nu = (long long)nx * upz;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long rows = (long long)r * nx, tot = std::max(rows * upz, (long long)nh);
+    static_pack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>((int)nz, (int)upz, rows, d_U, d_V, sU, sV, sOffs, nh, offs);
+    const long long quads = (long long)nx * (upz / 4);
+    gather_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(L, sU, sV, r, nh, sOffs, scale, d_gather);
+    CU(cudaGetLastError());
+    return RTM_OK;
+}
+
 extern "C" const char *rtm_strerror(int code) {
     switch (code) {
         case RTM_OK: return "ok";
@@ -1410,6 +1483,7 @@ extern "C" const char *rtm_strerror(int code) {
         case RTM_ENOMEM: return "workspace too small";
         case RTM_ECUDA: return "CUDA error";
         case RTM_ESTATE: return "call out of order";
+        case RTM_ELIMIT: return "size beyond the static scratch (RTM_STATIC_SCRATCH_BYTES / RTM_STATIC_MAX_OFFSETS in rtm.h)";
         default: return "unknown error";
     }
 }
