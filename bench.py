@@ -300,6 +300,8 @@ def run_ours(args):
         m.set_option("pdl", args.pdl)
         if args.rx and Tb > 1 and p.ndim == 2 and p.physics == 0:
             m.set_option("rx", args.rx)
+        if args.tti_tile and Tb > 8 and p.ndim == 2 and p.physics == 1:
+            m.set_option("tti_tile", args.tti_tile)
         m.set_probes(p.Z)
         return m
 
@@ -519,6 +521,7 @@ def main():
     ap.add_argument("--variants", type=int, default=1, help="also time the other probe variant (2 shots)")
     ap.add_argument("--pdl", type=int, default=1)
     ap.add_argument("--rx", type=int, default=0)
+    ap.add_argument("--tti-tile", type=int, default=0, help="2D TTI, time-blocked: rows per tile of the step kernel (16 | 32; 0 = the library's choice)")
     ap.add_argument("--nt", type=int, default=0, help="experiments only: shorten the record (not the headline config)")
     args = ap.parse_args()
     if args.impl == "reference":

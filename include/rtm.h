@@ -205,6 +205,8 @@ float rtm_pass_ms_mean(rtm_ctx *ctx, int which, int count);
  *                     launch-bound otherwise); 2: beyond that also one slab per SM exchanging rows through L2 (measured
  *                     slower than the streaming kernel at c1); 3: the L2 mode only; 0: never.  Same bits
  *                     in every mode.
+ *   "tti_tile"   16|32  2D TTI: rows per tile of the step kernel (256 or 512 threads per block).  32 (default when the time
+ *                     block has 9 .. 16 steps, the only case it exists for) recomputes less halo; same bits either way.
  * Errors: RTM_EINVAL (unknown name / value out of range).
  * Timing experiments that break the results ("dbg" masks, per-block time stamps) exist only in a library built with
  * -DRTM_DEBUG (see the end of this header); the product build has neither.                                */

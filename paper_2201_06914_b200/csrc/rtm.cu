@@ -85,6 +85,7 @@ struct rtm_ctx {
     float *k1x, *k1y, *k1z;
     float *Uz, *Vz, *Zf, *Za, *hist;
     int zr, T, rx;
+    int tti_tx;   // 2D TTI: rows per tile of tti_step_kernel, 16 (256 threads) or 32 (512 threads; time-blocked probing only)
     long long pNu;   // floats per history slot and per group of planes of one probe: Nu x probed fields
     int rp;   // probe planes per compressed array: r, or 2 r when p and r are probed apart (probe_fields = 2)
     int *row_start;
@@ -295,6 +296,7 @@ static int create_on_device(rtm_ctx *c, const rtm_config *cfg, void *d_workspace
     c->opt_pdl = 1;
     c->opt_dbg = 0;
     c->rx = (cfg->ndim == 2 && cfg->physics == 0 && c->T > 0) ? pick_rx(c) : 0;
+    c->tti_tx = (cfg->ndim == 2 && cfg->physics == 1 && tm_of(c->T) == 16) ? 32 : 16;
     c->ev_count[0] = c->ev_count[1] = 0;
     for (int i = 0; i < 2; i++)
         for (int s = 0; s < rtm_ctx::kEvRing; s++)
@@ -798,9 +800,9 @@ static void step_grid(const rtm_ctx *c, dim3 *grid, dim3 *block, size_t *smem) {
         *block = dim3(32, 8, 1);
         *smem = 0;
     } else if (c->cfg.physics == 1) {
-        *grid = dim3((L.Pz + TTI_TZ - 1) / TTI_TZ, (L.Px + TTI_TX - 1) / TTI_TX, 1);
-        *block = dim3(16, 16, 1);
-        *smem = std::max<size_t>((size_t)TTI_SMEM, (size_t)tm_of(c->T) * c->zr * 4);
+        *grid = dim3((L.Pz + TTI_TZ - 1) / TTI_TZ, (L.Px + c->tti_tx - 1) / c->tti_tx, 1);
+        *block = dim3(16, c->tti_tx, 1);
+        *smem = std::max<size_t>((size_t)tti_smem(c->tti_tx), (size_t)tm_of(c->T) * c->zr * 4);
     } else if (c->cfg.ndim == 2 && c->T > 0) {
         // streaming kernel: 1-D list of (row chunk, z-quad) tasks, 128 per block; grid.x = blocks,
         // a.gx is overwritten with the quads per row by run_pass
@@ -914,8 +916,11 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
                                  : launch_ex(c, tti_step_kernel<4>, a, nb, block, smem, st);
             case 8: return a.two ? launch_ex(c, tti_step_kernel<8, true>, a, nb, block, smem, st)
                                  : launch_ex(c, tti_step_kernel<8>, a, nb, block, smem, st);
-            default: return a.two ? launch_ex(c, tti_step_kernel<16, true>, a, nb, block, smem, st)
-                                  : launch_ex(c, tti_step_kernel<16>, a, nb, block, smem, st);
+            default:
+                if (c->tti_tx == 32) return a.two ? launch_ex(c, tti_step_kernel<16, true, 32>, a, nb, block, smem, st)
+                                                  : launch_ex(c, tti_step_kernel<16, false, 32>, a, nb, block, smem, st);
+                return a.two ? launch_ex(c, tti_step_kernel<16, true>, a, nb, block, smem, st)
+                             : launch_ex(c, tti_step_kernel<16>, a, nb, block, smem, st);
         }
     } else if (c->cfg.ndim == 2) {
         switch (tm) {
@@ -1392,6 +1397,12 @@ extern "C" int rtm_set_option(rtm_ctx *c, const char *name, int value) {
     if (!strcmp(name, "resident")) {   // 2D acoustic, T > 1: wavefield resident in shared memory for a whole time block
         if (value < 0 || value > 3) return RTM_EINVAL;
         c->opt_resident = value;
+        return RTM_OK;
+    }
+    if (!strcmp(name, "tti_tile")) {   // 2D TTI, time blocks of 9..16 steps: rows per tile of the step kernel, 16 or 32
+        if (c->cfg.ndim != 2 || c->cfg.physics != 1 || (value != 16 && value != 32)) return RTM_EINVAL;
+        if (value == 32 && tm_of(c->T) != 16) return RTM_EINVAL;   // the 32-row instance exists for T in 9..16 only
+        c->tti_tx = value;
         return RTM_OK;
     }
     if (!strcmp(name, "rx")) {   // rows per thread of the 2D streaming kernel (2|4|8|16); 0 = automatic

@@ -17,13 +17,17 @@
 
 namespace rtm {
 
-constexpr int TTI_TX = 16, TTI_TZ = 64;
-constexpr int TTI_FX = TTI_TX + 16, TTI_FZ = TTI_TZ + 16;   // field tile (halo 8)
-constexpr int TTI_GX = TTI_TX + 8, TTI_GZ = TTI_TZ + 8;     // product tile (halo 4)
-constexpr int TTI_SMEM = (2 * TTI_FX * TTI_FZ + 4 * TTI_GX * TTI_GZ) * 4;
+constexpr int TTI_TZ = 64;
+constexpr int TTI_FZ = TTI_TZ + 16;   // field tile (halo 8)
+constexpr int TTI_GZ = TTI_TZ + 8;    // product tile (halo 4)
+// Rows per tile: 16 (256 threads) or 32 (512 threads).  The halo recompute falls from 2.5 x / 1.69 x of the tile in stages
+// 1 / 2 to 1.875 x / 1.41 x with 32 rows, at the same 32 warps per SM (2 blocks of 512 threads and 77 KB instead of 4
+// blocks of 256 threads and 48 KB); the per-step fused variant (80 registers for the probe pipeline) keeps 16 rows.
+__host__ __device__ constexpr int tti_smem(int tx) { return (2 * (tx + 16) * TTI_FZ + 4 * (tx + 8) * TTI_GZ) * 4; }
 
-template <int TM, bool TWO = false>
-__global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const StepArgs a) {
+template <int TM, bool TWO = false, int TTI_TX = 16>
+__global__ void __launch_bounds__(16 * TTI_TX, TM == 0 ? 3 : (TTI_TX == 16 ? 4 : 2)) tti_step_kernel(const StepArgs a) {
+    constexpr int TTI_FX = TTI_TX + 16, TTI_GX = TTI_TX + 8, NT = 16 * TTI_TX;
     extern __shared__ __align__(16) float smem[];
     float *sA = smem;                          // [FX][FZ]
     float *sB = sA + TTI_FX * TTI_FZ;
@@ -37,51 +41,79 @@ __global__ void __launch_bounds__(256, TM == 0 ? 3 : 4) tti_step_kernel(const St
     if (TM == 0) pdl_launch_dependents();
     if (TM > 0 && blockIdx.x < (unsigned)a.fl_blocks) {
         pdl_launch_dependents();
-        flush_role<(TM > 0 ? TM : 1)>(a, smem, tid, 256, blockIdx.x);
+        flush_role<(TM > 0 ? TM : 1)>(a, smem, tid, NT, blockIdx.x);
         return;
     }
     pdl_wait();
     if (TM > 0) pdl_launch_dependents();   // only now: lets the next step's flush role run without a wait (see flush_role)
     const unsigned lin_block = blockIdx.x - (TM > 0 ? a.fl_blocks : 0);
-    sample_points(a, lin_block, 256, tid);
+    sample_points(a, lin_block, NT, tid);
 
     const int z0 = (lin_block % a.gx) * TTI_TZ, x0 = (lin_block / a.gx) * TTI_TX;
 
     // ---- stage 1: (mixed) fields, halo 8 ----
-    for (int i = tid; i < TTI_FX * (TTI_FZ / 4); i += 256) {
-        const int lx = i / (TTI_FZ / 4), lq = i % (TTI_FZ / 4);
-        const int jx = x0 - 8 + lx, jz = z0 - 8 + lq * 4;
-        float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;
-        if (jx < L.Px + 8 && jz + 3 < L.pz - 8) {
-            const long long o = L.org + jx * L.sx + jz;
-            va = ld4(a.u0 + o);
-            vb = ld4(a.u1 + o);
-            if (a.adjoint) {
-                const float4 e = ld4(a.epsh + o), d = ld4(a.delh + o);
-                float4 ma, mb;
-                ma.x = fmaf(e.x, va.x, d.x * vb.x); mb.x = fmaf(d.x, va.x, vb.x);
-                ma.y = fmaf(e.y, va.y, d.y * vb.y); mb.y = fmaf(d.y, va.y, vb.y);
-                ma.z = fmaf(e.z, va.z, d.z * vb.z); mb.z = fmaf(d.z, va.z, vb.z);
-                ma.w = fmaf(e.w, va.w, d.w * vb.w); mb.w = fmaf(d.w, va.w, vb.w);
-                va = ma; vb = mb;
+    // All loads of a thread's N1 quads are issued before the first one is used: the stage is a single round trip to
+    // L2 / DRAM per block instead of one per loop iteration (the fields do not all stay in L2 beside the probe stream).
+    constexpr int N1 = (TTI_FX * (TTI_FZ / 4) + NT - 1) / NT;
+    {
+        float4 va[N1], vb[N1], ve[N1], vd[N1];
+        int so[N1];
+#pragma unroll
+        for (int k = 0; k < N1; k++) {
+            const int i = tid + k * NT;
+            const int lx = i / (TTI_FZ / 4), lq = i % (TTI_FZ / 4);
+            const int jx = x0 - 8 + lx, jz = z0 - 8 + lq * 4;
+            so[k] = i < TTI_FX * (TTI_FZ / 4) ? lx * TTI_FZ + lq * 4 : -1;
+            va[k] = make_float4(0.f, 0.f, 0.f, 0.f); vb[k] = va[k]; ve[k] = va[k]; vd[k] = va[k];
+            if (so[k] >= 0 && jx < L.Px + 8 && jz + 3 < L.pz - 8) {
+                const long long o = L.org + jx * L.sx + jz;
+                va[k] = ld4(a.u0 + o);
+                vb[k] = ld4(a.u1 + o);
+                if (a.adjoint) { ve[k] = ld4(a.epsh + o); vd[k] = ld4(a.delh + o); }
             }
         }
-        st4(sA + lx * TTI_FZ + lq * 4, va);
-        st4(sB + lx * TTI_FZ + lq * 4, vb);
+#pragma unroll
+        for (int k = 0; k < N1; k++) {
+            if (so[k] < 0) continue;
+            float4 xa = va[k], xb = vb[k];
+            if (a.adjoint) {
+                const float4 e = ve[k], d = vd[k];
+                float4 ma, mb;
+                ma.x = fmaf(e.x, xa.x, d.x * xb.x); mb.x = fmaf(d.x, xa.x, xb.x);
+                ma.y = fmaf(e.y, xa.y, d.y * xb.y); mb.y = fmaf(d.y, xa.y, xb.y);
+                ma.z = fmaf(e.z, xa.z, d.z * xb.z); mb.z = fmaf(d.z, xa.z, xb.z);
+                ma.w = fmaf(e.w, xa.w, d.w * xb.w); mb.w = fmaf(d.w, xa.w, xb.w);
+                xa = ma; xb = mb;
+            }
+            st4(sA + so[k], xa);
+            st4(sB + so[k], xb);
+        }
+    }
+    // cos / sin of this thread's stage-2 quads: requested before the barrier, so that their latency overlaps with it
+    constexpr int N2 = (TTI_GX * (TTI_GZ / 4) + NT - 1) / NT;
+    float4 csv[N2], snv[N2];
+#pragma unroll
+    for (int k = 0; k < N2; k++) {
+        const int i = tid + k * NT;
+        const int lx = i / (TTI_GZ / 4), lq = i - lx * (TTI_GZ / 4);
+        const int jx = x0 - 4 + lx, jz = z0 - 4 + lq * 4;
+        csv[k] = make_float4(0.f, 0.f, 0.f, 0.f); snv[k] = csv[k];
+        if (i < TTI_GX * (TTI_GZ / 4) && jx < L.Px + 8 && jz + 3 < L.pz - 8) {
+            const long long o = L.org + jx * L.sx + jz;
+            csv[k] = ld4(a.cs + o);
+            snv[k] = ld4(a.sn + o);
+        }
     }
     __syncthreads();
 
     // ---- stage 2: rotated gradients times cos / sin, halo 4; one z-quad per thread and round ----
     // centred first derivative of a quad: x from the 8 neighbour rows (LDS.128 each), z from the 12-float window
-    for (int i = tid; i < TTI_GX * (TTI_GZ / 4); i += 256) {
+#pragma unroll
+    for (int k = 0; k < N2; k++) {
+        const int i = tid + k * NT;
+        if (i >= TTI_GX * (TTI_GZ / 4)) break;
         const int lx = i / (TTI_GZ / 4), lq = i - lx * (TTI_GZ / 4);
-        const int jx = x0 - 4 + lx, jz = z0 - 4 + lq * 4;
-        float4 cs4 = make_float4(0.f, 0.f, 0.f, 0.f), sn4 = cs4;
-        if (jx < L.Px + 8 && jz + 3 < L.pz - 8) {
-            const long long o = L.org + jx * L.sx + jz;
-            cs4 = ld4(a.cs + o);
-            sn4 = ld4(a.sn + o);
-        }
+        const float4 cs4 = csv[k], sn4 = snv[k];
         const float *fa = sA + (lx + 4) * TTI_FZ + (lq * 4 + 4);
         const float *fb = sB + (lx + 4) * TTI_FZ + (lq * 4 + 4);
         float ax[4] = {0.f, 0.f, 0.f, 0.f}, bx[4] = {0.f, 0.f, 0.f, 0.f};

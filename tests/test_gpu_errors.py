@@ -181,4 +181,18 @@ def test_option_values_are_validated():
     m3 = _mk(ri.random_acoustic(3, n=(14, 12, 10), nb=4, nt=5, r=2), probe_block=8)
     with pytest.raises(RTMError):
         m3.set_option("rx", 4)                      # the 2D streaming kernel's knob
+    with pytest.raises(RTMError):
+        m3.set_option("tti_tile", 16)               # the 2D TTI kernel's knob
     m3.close()
+    q = ri.random_tti(n=(40, 36), nb=8, nt=10, r=3, seed=2)
+    mt = _mk(q, probe_block=16)
+    for bad in (0, 8, 24, 64):
+        with pytest.raises(RTMError):
+            mt.set_option("tti_tile", bad)
+    mt.set_option("tti_tile", 16)
+    mt.set_option("tti_tile", 32)
+    mt.close()
+    mt = _mk(q, probe_block=8)                      # the 32-row instance exists for time blocks of 9 .. 16 steps
+    with pytest.raises(RTMError):
+        mt.set_option("tti_tile", 32)
+    mt.close()

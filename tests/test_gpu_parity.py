@@ -48,6 +48,26 @@ def test_tti_random_offgrid(n, nb, r):
     check_all(p, snap_steps=[10, 40, 79], offsets=np.array([-1, 0, 4], np.int32))
 
 
+def test_tti_tile_rows_do_not_change_a_bit():
+    """tti_step_kernel with 16 or 32 rows per tile (option "tti_tile"; 32 is the default for T in 9..16): same
+    operations per point in the same order, so every output is bit-identical; grid with ragged tiles in x and z."""
+    from paper_2201_06914_b200 import Rtm
+    p = ri.random_tti(n=(75, 131), nb=12, nt=60, r=7, seed=6, nsrc=2, nrec=6)
+    outs = []
+    for rows in (16, 32):
+        m = Rtm.from_problem(p, probe_block=16)
+        m.set_option("tti_tile", rows)
+        m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta)
+        m.set_probes(p.Z)
+        d = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+        img, q = m.adjoint_image(p.rec_xyz, d, p.src_xyz, qadj_out=True)
+        outs.append([x.cpu().numpy() for x in (d, img, q, m.export_probes(0), m.export_probes(1))])
+        m.close()
+    assert np.abs(outs[0][1]).max() > 0
+    for x, y in zip(outs[0], outs[1]):
+        assert np.array_equal(x, y)
+
+
 @pytest.mark.parametrize("nb", [1, 2, 3, 5, 6, 7])
 def test_layer_thickness_need_not_be_a_multiple_of_4(nb):
     """Any nb: the internal z axis starts (4 - nb % 4) % 4 points before the padded grid (K2 = 0 there) so that the
