@@ -50,9 +50,9 @@ def test_c1_full_shot_against_oracle():
 def test_tti_long_record():
     """3000 steps of 2D TTI on a 400 x 300 crop of c2 (time-blocked T = 16, the 32-row tile kernel): every output inside
     the standard tolerances.  Longer TTI records drift out of them in the forward compressed wavefield (DESIGN.md,
-    "Long 2D TTI records": rounding errors that land in the Nyquist null space of the centred rotated operator have no
-    restoring force; Uz 9.6e-5 at 4000 steps, 4.9e-4 at 8000 on this crop); this case catches a change that makes the
-    drift worse."""
+    "Long 2D TTI records": rounding errors that land in the stationary branch of the pseudo-acoustic system where
+    eps = delta, or in the Nyquist null space of the centred rotated operator, have no restoring force; Uz 9.6e-5 at 4000
+    steps, 4.9e-4 at 8000 on this crop); this case catches a change that makes the drift worse."""
     p = ri.make_c2(n=(400, 300), nt=3000, r=8, nb=40)
     offs = np.array([-20, 0, 7], np.int32)
     g = run_gpu(p, offsets=offs, probe_block=16)
