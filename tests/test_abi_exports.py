@@ -145,3 +145,26 @@ def test_qr_probes_host_match_oracle():
     with pytest.raises(RTMError) as e:                       # r > nt
         probes_qr_host(rng.standard_normal((4, 9)).astype(np.float32), np.ones((4, 6), np.float32))
     assert e.value.code == -1
+
+
+def test_static_gather_argument_checks_need_no_device():
+    """rtm_offset_gather_static validates sizes against the static scratch (rtm.h: RTM_STATIC_SCRATCH_BYTES,
+    RTM_STATIC_MAX_OFFSETS) before it touches CUDA, so the checks run here: no launch happens on any of these paths."""
+    import ctypes as C
+    _build()
+    from paper_2201_06914_b200 import binding as B
+    lib = B.load_library()
+    fake = C.c_void_p(256)            # never dereferenced: every call below returns before any CUDA call
+    offs = (C.c_int * 80)(*([0] * 80))
+    call = lambda nx, nz, r, nh, U=fake, V=fake, G=fake, o=offs: lib.rtm_offset_gather_static(
+        nx, nz, r, U, V, nh, C.cast(o, C.c_void_p), C.c_float(1.0), G, None)
+    assert call(16, 12, 2, 65) == -5                                  # more than RTM_STATIC_MAX_OFFSETS
+    r, nz = 2, 1024
+    nx_max = (B.STATIC_SCRATCH_BYTES - 256) // (2 * r * nz * 4)
+    assert call(nx_max + 1, nz, r, 1) == -5                           # one row beyond the static array
+    assert call(1 << 30, 1 << 30, 1 << 30, 1) == -5                   # no overflow in the size check
+    assert call(0, 12, 2, 1) == -1 and call(16, 12, 0, 1) == -1 and call(16, 12, 2, 0) == -1
+    assert call(16, 12, 2, 1, U=None) == -1 and call(16, 12, 2, 1, G=None) == -1
+    bad = (C.c_int * 80)(*([16] + [0] * 79))
+    assert call(16, 12, 2, 1, o=bad) == -1                            # |h| >= nx
+    assert b"static scratch" in lib.rtm_strerror(-5)
