@@ -129,8 +129,9 @@ def propagate(p, co: Coeffs, adjoint: bool, inj_xyz, inj_val, smp_xyz=None, Z=No
     ss = np.asarray(list(snap_steps), np.int32)
     snaps = np.zeros((len(ss), nf, Np), np.float64) if len(ss) else None
     if p.physics == 1 and p.ndim == 3:
-        assert fields == 1 and co.cosP is not None
-        rc = lib.orc_propagate3(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
+        assert co.cosP is not None
+        fn3 = lib.orc_propagate3 if fields == 1 else lib.orc_propagate3_pr      # readings C30 / C29 + C30
+        rc = fn3(C.byref(c), C.c_int(1 if adjoint else 0), _fp(co.K2), _fp(co.damp), _fp(co.epsh),
                                 _fp(co.delh), _fp(co.cosT), _fp(co.sinT), _fp(co.cosP), _fp(co.sinP), C.c_int(ninj),
                                 _fp(inj_xyz), _fp(inj_val), C.c_int(nsmp), _fp(smp_xyz), _fp(out), _fp(Zc), _fp(PZ),
                                 _fp(hist), C.c_int(len(ss)), _fp(ss), _fp(snaps))

@@ -30,6 +30,8 @@
  * VTI is faster along x by sqrt(1 + 2 eps); with theta = +30 deg the fast direction is (cos th, -sin th).
  * 3D TTI (C30; tests/test_oracle_tti3d.py): dot test, H symmetric negative semi-definite, H_perp + H_par = Laplacian for
  * constant angles, eps = delta = 0 => p == r == acoustic, tilted kinematics (c along n, c sqrt(1+2 eps) along e1, e2).
+ * Two probed fields in 3D (C29 + C30): 1/2 (Pz + Rz) == the one-field planes, PZ == hist^T Z by numpy per field, history
+ * field 0 / 1 == physical part of the p / r snapshot.
  * PARITY UNPINNED (free choices no external fact fixes; the implementation is pinned to its stated design, the
  * design itself is a choice): the damping profile shape and strength, the wavelet delay, and imaging the single
  * TTI field (p+r)/2.
@@ -573,6 +575,17 @@ int orc_propagate_pr(const orc_cfg *c, int adjoint, const float *K2, const float
                      int nsnap, const int *snap_steps, double *snaps) {
     return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, NULL, NULL, ninj, inj_xyz, inj_val, nsmp, smp_xyz, smp_out,
                      Z, PZ, hist, nsnap, snap_steps, snaps, 2);
+}
+
+/* The same four arrays for 3D TTI (readings C29 + C30: Eq. 2-3, on the (p, r) system of L77 in the 3D
+ * form of L81): orc_propagate3 with p and r probed apart, PZ [2][r][N], hist [nt][2][N].                        */
+int orc_propagate3_pr(const orc_cfg *c, int adjoint, const float *K2, const float *damp,
+                      const float *epsh, const float *delh, const float *cosT, const float *sinT, const float *cosP,
+                      const float *sinP, int ninj, const float *inj_xyz, const float *inj_val, int nsmp,
+                      const float *smp_xyz, double *smp_out, const float *Z, double *PZ /*[2][r][N]*/,
+                      double *hist /*[nt][2][N]*/, int nsnap, const int *snap_steps, double *snaps) {
+    return propagate(c, adjoint, K2, damp, epsh, delh, cosT, sinT, cosP, sinP, ninj, inj_xyz, inj_val, nsmp, smp_xyz,
+                     smp_out, Z, PZ, hist, nsnap, snap_steps, snaps, 2);
 }
 
 /* ==== O4. Images ============================================================================== */

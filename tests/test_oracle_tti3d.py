@@ -137,3 +137,34 @@ def test_tilted_3d_kinematics():
     assert abs(v["axis"] - 1.0) <= 1e-2, v
     assert abs(v["e1"] / fast - 1.0) <= 1e-2 and abs(v["e2"] / fast - 1.0) <= 1e-2, v
     assert v["e1_mirror"] < 1.08 and v["e2_mirror"] < 1.16, v       # 30 deg / 60 deg off the axis: clearly slower than e1, e2
+
+
+def test_two_probed_fields_3d():
+    """Readings C29 + C30 (four compressed arrays of the TTI gradient, in 3D): with fields = 2 the pass probes p and r
+    apart.  Pinned against things the one-field pass and numpy already fix: (i) plane k of p plus plane k of r, halved,
+    is the one-field plane of 1/2 (p + r); (ii) PZ = hist^T Z by a numpy matmul, field by field; (iii) field 0 of the
+    history is the physical part of the p snapshot and field 1 of the r snapshot (kills a swap of the two)."""
+    p = ri.random_tti3d(n=(13, 11, 12), nb=4, nt=30, r=3, seed=5)
+    co = orc.coeffs(p)
+    one = orc.forward(p, co, Z=p.Z)
+    steps = [7, 29]
+    two = orc.forward(p, co, Z=p.Z, fields=2, want_hist=True, snap_steps=steps)
+    P, R = two["PZ"][:p.r], two["PZ"][p.r:]
+    assert np.abs(one["PZ"]).max() > 0 and np.abs(P - R).max() > 1e-3 * np.abs(P).max()      # p and r do differ
+    assert np.abs(0.5 * (P + R) - one["PZ"]).max() <= 1e-12 * np.abs(one["PZ"]).max()
+    assert np.array_equal(two["samples"], one["samples"])
+    Z = p.Z.astype(np.float64)
+    for f in range(2):
+        ref = Z.T @ two["hist"][:, f, :]
+        assert np.abs(ref - two["PZ"][f * p.r:(f + 1) * p.r]).max() <= 1e-12 * np.abs(ref).max()
+    nb = p.nb
+    for q, n in enumerate(steps):
+        for f in range(2):
+            full = two["snaps"][q, f].reshape(p.P)
+            phys = full[nb:nb + p.n[0], nb:nb + p.n[1], nb:nb + p.n[2]].ravel()
+            assert np.array_equal(phys, two["hist"][n, f])
+    # the adjoint pass takes the same path
+    d = one["samples"].astype(np.float32)
+    a1 = orc.adjoint(p, co, d, Z=p.Z)
+    a2 = orc.adjoint(p, co, d, Z=p.Z, fields=2)
+    assert np.abs(0.5 * (a2["PZ"][:p.r] + a2["PZ"][p.r:]) - a1["PZ"]).max() <= 1e-12 * np.abs(a1["PZ"]).max()
