@@ -56,7 +56,7 @@ typedef struct {
                        Same sums, same order per (k,x); costs 2 T_b N floats of workspace (the ring is
                        double-buffered: one half is filled while the other is flushed).             */
     int probe_fields;/* 0|1: one probed field per pass (TTI: 1/2 (p + r), reading C10).
-                       2 (physics 1 only; any probe_block): the exact TTI gradient's four compressed arrays
+                       2 (physics 1 only, 2D and 3D; any probe_block): the exact TTI gradient's four compressed arrays
                        (Eq. 2-3, on the coupled (p, r) system of L77; reading C29): every pass probes
                        p and r apart with the same Z, Uz = (Pz, Rz), Vz = (Wpz, Wrz), 2r planes each; the image and
                        the gathers sum over the 2r planes, scale = 1/r; rtm_export_probes returns [2r][N] (p planes, then

@@ -140,7 +140,7 @@ static bool valid_cfg(const rtm_config *c) {
     if (c->probe_block > 16 && c->r > 128) return false;   // staging of the 32 Z rows in the final flush kernel
     // four compressed arrays for the TTI gradient (reading C29): TTI only
     if (c->probe_fields != 0 && c->probe_fields != 1 && c->probe_fields != 2) return false;
-    if (c->probe_fields == 2 && (c->physics != 1 || c->ndim != 2)) return false;
+    if (c->probe_fields == 2 && c->physics != 1) return false;
     return true;
 }
 
@@ -907,6 +907,7 @@ static int launch_step(rtm_ctx *c, const StepArgs &a, dim3 grid, dim3 block, siz
         int rc = 0;
         if (a.adjoint && (rc = launch_ex(c, tti3d_mix_kernel, a, nb, block, 0, st))) return rc;
         if ((rc = launch_ex(c, tti3d_grad_kernel, a, nb, block, 0, st))) return rc;
+        if (a.two) return tm == 0 ? launch_ex(c, tti3d_step_kernel<0, true>, a, nb, block, 0, st) : launch_ex(c, tti3d_step_kernel<16, true>, a, nb, block, 0, st);
         return tm == 0 ? launch_ex(c, tti3d_step_kernel<0>, a, nb, block, 0, st) : launch_ex(c, tti3d_step_kernel<16>, a, nb, block, 0, st);
     } else if (c->cfg.physics == 1) {
         switch (tm) {

@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) tti3d_grad_kernel(const StepArgs a) {
     for (int k = 0; k < 6; k++) st4(a.F[k] + o, make_float4(F[k][0], F[k][1], F[k][2], F[k][3]));
 }
 
-template <int TM>
+template <int TM, bool TWO = false>
 __global__ void __launch_bounds__(256, 2) tti3d_step_kernel(const StepArgs a) {
     pdl_launch_dependents();
     pdl_wait();
@@ -167,9 +167,19 @@ __global__ void __launch_bounds__(256, 2) tti3d_step_kernel(const StepArgs a) {
     const int ix = jx - L.nb, iy = jy - L.nby, iz = jz - L.nbz;
     if (ix >= 0 && ix < L.nx && iy >= 0 && iy < L.ny && iz >= 0 && iz < L.nz) {
         const long long o = ((long long)ix * L.ny + iy) * L.upz + iz;
-        const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
-        if (TM > 0) { if (a.hist != nullptr) stcs4(a.hist + o, v); }
-        else if (a.PZ != nullptr) probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+        if (!TWO) {
+            const float4 v = make_float4(pr[0], pr[1], pr[2], pr[3]);
+            if (TM > 0) { if (a.hist != nullptr) stcs4(a.hist + o, v); }
+            else if (a.PZ != nullptr) probe_quad<2>(a.PZ + o, L.Nu, a.Zrow, a.r, v);
+        } else {
+            // p and r probed apart (readings C29 + C30), laid out as in tti.cuh: plane (or history half-slot) 2k = p, 2k + 1 = r
+            const float4 wp = make_float4(pn[0], pn[1], pn[2], pn[3]), wr = make_float4(rn[0], rn[1], rn[2], rn[3]);
+            if (TM > 0) {
+                if (a.hist != nullptr) { stcs4(a.hist + o, wp); stcs4(a.hist + L.Nu + o, wr); }
+            } else if (a.PZ != nullptr) {
+                for (int f = 0; f < 2; f++) probe_quad<2>(a.PZ + (long long)f * L.Nu + o, 2 * L.Nu, a.Zrow, a.r, f ? wr : wp);
+            }
+        }
     }
 }
 

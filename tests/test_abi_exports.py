@@ -104,7 +104,10 @@ def test_host_coefficients_3d_tti_match_oracle_bitwise():
     co = orc.coeffs(p)
     for a, b in ((K2, co.K2), (damp, co.damp), (eh, co.epsh), (dh, co.delh), (cs, co.cosT), (sn, co.sinT), (cp, co.cosP), (sp, co.sinP)):
         assert np.array_equal(a, b)
-    assert B.workspace_bytes(B.make_config(3, p.n, p.h, p.nb, 1, p.nt, p.dt, p.r, 8, probe_fields=2)) == 0    # four-array mode: 2D TTI only
+    one = B.workspace_bytes(B.make_config(3, p.n, p.h, p.nb, 1, p.nt, p.dt, p.r, 8))
+    two = B.workspace_bytes(B.make_config(3, p.n, p.h, p.nb, 1, p.nt, p.dt, p.r, 8, probe_fields=2))
+    assert two > one > 0                                                     # four-array mode: TTI in 2D and 3D, twice the planes
+    assert B.workspace_bytes(B.make_config(3, p.n, p.h, p.nb, 0, p.nt, p.dt, p.r, 8, probe_fields=2)) == 0    # not for acoustic physics
 
 
 def test_coeffs_host_rejects_bad_time_step_and_spacing():

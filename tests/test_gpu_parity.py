@@ -444,6 +444,50 @@ def test_tti_gradient_with_four_compressed_arrays(n, nt, r, T):
             assert rel(img, Iex) <= 1e-4, rel(img, Iex)
 
 
+@pytest.mark.parametrize("n,nb,r,T", [((20, 18, 22), 6, 4, 0), ((37, 19, 40), 5, 3, 16)])
+def test_tti3d_gradient_with_four_compressed_arrays(n, nb, r, T):
+    """Readings C29 + C30: probe_fields = 2 on a 3D TTI context (p and r probed apart, per-step fused and time-blocked with
+    nt not a multiple of T) -- planes, image and gather against orc_propagate3_pr; data and adjoint traces are the
+    one-field run's bit for bit; the p and r planes are not swapped."""
+    import oracle as orc
+    from paper_2201_06914_b200 import Rtm, probes_dtt_host
+    p = ri.random_tti3d(n=n, nb=nb, nt=45, r=r, seed=6, nsrc=2, nrec=6)
+    co = orc.coeffs(p)
+    one = run_gpu(p, probe_block=T)
+    offs = np.array([-2, 0, 1], np.int32)
+    Zdd = probes_dtt_host(p.Z, p.dt)
+    m = Rtm.from_problem(p, probe_fields=2, probe_block=T)
+    m.set_model_from_earth(p.vp, p.eps, p.delta, p.theta, p.phi)
+    m.set_probes(Zdd, p.Z)
+    data = m.forward_probe(p.src_xyz, p.wav, p.rec_xyz).cpu().numpy()
+    assert np.array_equal(data, one["data"])
+    img, q = m.adjoint_image(p.rec_xyz, data, p.src_xyz, qadj_out=True)
+    assert np.array_equal(q.cpu().numpy(), one["qadj"])
+    Uz, Vz = m.export_probes(0).cpu().numpy(), m.export_probes(1).cpu().numpy()
+    assert Uz.shape == (2 * r, p.N)
+    img = img.cpu().numpy().ravel()
+    gat = m.offset_gather(offs).cpu().numpy().reshape(len(offs), -1)
+    m.close()
+    f = orc.forward(p, co, Z=Zdd, fields=2)
+    a = orc.adjoint(p, co, data, Z=p.Z, fields=2)
+    I = orc.image(f["PZ"], a["PZ"], 1.0 / r)
+    G = orc.offset_gather(p.n, f["PZ"], a["PZ"], offs, 1.0 / r)
+    errs = {"Pz": rel(Uz[:r], f["PZ"][:r]), "Rz": rel(Uz[r:], f["PZ"][r:]), "Wpz": rel(Vz[:r], a["PZ"][:r]),
+            "Wrz": rel(Vz[r:], a["PZ"][r:]), "image": rel(img, I), "gather": rel(gat, G)}
+    print(n, T, {k: "%.2e" % v for k, v in errs.items()})
+    assert np.abs(I).max() > 0 and max(errs.values()) <= 1e-4, errs
+    assert np.array_equal(gat[1], img)                                       # PAPER.md:L52
+    assert rel(Uz[:r], f["PZ"][r:]) > 1e-3                                   # p and r planes are not swapped
+    # the one-field planes of 1/2 (p + r) with the same probes, from the two-field planes (fp32 rounding apart)
+    m1 = Rtm.from_problem(p, probe_block=T)
+    m1.set_model_from_earth(p.vp, p.eps, p.delta, p.theta, p.phi)
+    m1.set_probes(Zdd, p.Z)
+    m1.forward_probe(p.src_xyz, p.wav, p.rec_xyz)
+    U1 = m1.export_probes(0).cpu().numpy()
+    m1.close()
+    assert rel(0.5 * (Uz[:r].astype(np.float64) + Uz[r:]), U1) <= 1e-5
+
+
 def test_four_array_mode_is_for_tti_and_does_not_depend_on_the_time_block():
     from paper_2201_06914_b200 import Rtm, RTMError, probes_dtt_host
     pa = ri.random_acoustic(2, n=(30, 28), nb=4, nt=10, r=2)
